@@ -1,0 +1,207 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.  Not part of the product path.
+//
+// Plain, slow, obviously-correct FP64 CPU implementation of direct inverse ray-shooting (GERLUMPH / GPU-D hot path,
+// Vernardos & Fluke 2014, arXiv:1406.0559).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference legs may load this library.  It shares NO code with the CUDA path (paper_1406_0559_b200/csrc):
+// no headers, helpers, tables or constants.
+//
+// What it follows, in the paper's order and notation:
+//   * PAPER.md:71   "large numbers (~10^9) of light rays are projected from the observer, through the lens plane,
+//                    where they are each deflected by N_* individual lenses ... and accumulated on a gridded source
+//                    plane"                                                        -> the three nested loops below
+//   * PAPER.md:73   Eq. (1)  y = diag(1-gamma, 1+gamma) x - kappa_s x - sum_i m_i (x - x_i)/|x - x_i|^2
+//   * PAPER.md:75-77 Eq. (2) kappa = kappa_s + kappa_*,  s = kappa_s/kappa
+//   * PAPER.md:85-87 Eq. (4) mu_ij = N_ij / N_avg
+//   * PAPER.md:103  Fig. 1: regular grid of rays on the lens plane; rectangular pixellated source-plane area.
+// Where the paper is silent the readings S1-S17 of SURVEY.md §8(c) (restated in DESIGN.md "Readings") apply:
+//   S2 cell-centred symmetric lattice  x = (i + 1/2 - n/2) d,  n = 2*ceil(a/d - 1e-9),
+//      a1 = 1.2 (L/2)/|1-kappa-gamma|, a2 = 1.2 (L/2)/|1-kappa+gamma|          (BASELINE.json config rule)
+//   S4 half-open pixels, floor; ix from y1, iy from y2; row-major iy*Npix+ix; corner of pixel (0,0) at (-L/2,-L/2)
+//   S5 N_avg = (p/d)^2                                                            (BASELINE.json north_star)
+//   S7 no softening; a non-finite source position counts as "lost" and is not binned
+//   S8 lenses summed in input order, one FP64 accumulator per component
+//   S14 lens arrays are FP32 at the interface and promoted exactly to double
+//   S16 mag = (float)((double)count / N_avg)
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 no-lens closed form, P2 single point lens A(u), P3 hand sums
+// (tests/golden/p3_hand_sums.txt), P4 ray conservation, P5 mean magnification, P6 mirror symmetry, P7 lens-order
+// permutation, P8 mass-sheet transformation.  Parity status: pinned (the dense many-caustic regime itself has no
+// closed form; there this code path, anchored by P1-P8, is the reference).
+//
+// Build: g++ -O3 -march=native -fopenmp -shared -fPIC oracle/oracle.cpp -o oracle/liboracle.so   (no fast-math)
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+
+struct oracle_geometry {
+    long long n1, n2;                       // lattice counts along x1, x2
+    double a1, a2;                          // rectangle half-widths
+    double p, d;                            // pixel size, ray spacing
+    double kappa_s, kappa_star, n_avg;      // Eq. 2 split; N_avg = (p/d)^2
+};
+
+struct oracle_stats {
+    long long rays_total, rays_in_map, rays_outside, rays_lost;
+};
+
+// Derived quantities (readings S2, S5).  Returns 0, or -1 on the critical line / bad arguments.
+int oracle_derive_geometry(double kappa, double gamma, double s, double L, int npix, double d, oracle_geometry* g) {
+    if (!(L > 0) || npix <= 0 || !(d > 0) || !(s >= 0 && s <= 1)) return -1;
+    const double f1 = std::fabs(1.0 - kappa - gamma), f2 = std::fabs(1.0 - kappa + gamma);
+    if (f1 < 1e-6 || f2 < 1e-6) return -1;
+    g->kappa_s = s * kappa;
+    g->kappa_star = kappa - g->kappa_s;
+    g->p = L / npix;
+    g->d = d;
+    g->a1 = 1.2 * (L / 2.0) / f1;
+    g->a2 = 1.2 * (L / 2.0) / f2;
+    g->n1 = 2 * (long long)std::ceil(g->a1 / d - 1e-9);
+    g->n2 = 2 * (long long)std::ceil(g->a2 / d - 1e-9);
+    g->n_avg = (g->p / d) * (g->p / d);
+    return 0;
+}
+
+// One ray, Eq. (1) written out.  alpha = sum_i m_i (x - x_i)/|x - x_i|^2 ; scale = sum_i m_i/|x - x_i| (the
+// north_star's tolerance scale for the per-ray deflection check).
+static inline void shoot_one(double x1, double x2, double kappa_s, double gamma, const float* lens_xy,
+                             const float* lens_m, long long n_lens, double* y1, double* y2, double* al1, double* al2,
+                             double* scale /* NULL: skip the sqrt */) {
+    double a1s = 0.0, a2s = 0.0, sc = 0.0;
+    for (long long k = 0; k < n_lens; ++k) {
+        const double dx = x1 - (double)lens_xy[2 * k];
+        const double dy = x2 - (double)lens_xy[2 * k + 1];
+        const double r2 = dx * dx + dy * dy;
+        const double m = lens_m ? (double)lens_m[k] : 1.0;
+        const double w = m / r2;
+        a1s += w * dx;
+        a2s += w * dy;
+        if (scale) sc += m / std::sqrt(r2);
+    }
+    *y1 = (1.0 - kappa_s - gamma) * x1 - a1s;
+    *y2 = (1.0 - kappa_s + gamma) * x2 - a2s;
+    *al1 = a1s;
+    *al2 = a2s;
+    if (scale) *scale = sc;
+}
+
+// Pixel id of a source position: >= 0 in map, -1 outside, -2 non-finite (readings S4, S7).
+static inline int pixel_of(double y1, double y2, double L, double p, int npix) {
+    if (!std::isfinite(y1) || !std::isfinite(y2)) return -2;
+    const double u1 = (y1 + L / 2.0) / p;
+    const double u2 = (y2 + L / 2.0) / p;
+    if (u1 >= 0.0 && u1 < (double)npix && u2 >= 0.0 && u2 < (double)npix)
+        return (int)std::floor(u2) * npix + (int)std::floor(u1);
+    return -1;
+}
+
+// Rays i0 <= i < i0+ni, j0 <= j < j0+nj of the lattice.  count (npix*npix int32) is ACCUMULATED into (may be NULL).
+// Optional per-ray outputs, ray (ii, jj) of the block at index q = jj*ni + ii:
+//   ray_y[2q], ray_y[2q+1] source position; ray_alpha[2q..] deflection; ray_scale[q]; ray_pix[q].
+int oracle_shoot_block(double kappa, double gamma, double s, double L, int npix, double d, const float* lens_xy,
+                       const float* lens_m, long long n_lens, long long i0, long long j0, long long ni, long long nj,
+                       int* count, double* ray_y, double* ray_alpha, double* ray_scale, int* ray_pix,
+                       oracle_stats* stats, int n_threads) {
+    oracle_geometry g;
+    if (oracle_derive_geometry(kappa, gamma, s, L, npix, d, &g) != 0) return -1;
+    if (i0 < 0 || j0 < 0 || ni < 0 || nj < 0 || i0 + ni > g.n1 || j0 + nj > g.n2) return -1;
+    long long in_map = 0, outside = 0, lost = 0;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : in_map, outside, lost)
+    for (long long jj = 0; jj < nj; ++jj) {
+        const double x2 = ((double)(j0 + jj) + 0.5 - (double)g.n2 / 2.0) * d;
+        for (long long ii = 0; ii < ni; ++ii) {
+            const double x1 = ((double)(i0 + ii) + 0.5 - (double)g.n1 / 2.0) * d;
+            double y1, y2, al1, al2, sc = 0.0;
+            shoot_one(x1, x2, g.kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, ray_scale ? &sc : nullptr);
+            const int pix = pixel_of(y1, y2, L, g.p, npix);
+            const long long q = jj * ni + ii;
+            if (ray_y) { ray_y[2 * q] = y1; ray_y[2 * q + 1] = y2; }
+            if (ray_alpha) { ray_alpha[2 * q] = al1; ray_alpha[2 * q + 1] = al2; }
+            if (ray_scale) ray_scale[q] = sc;
+            if (ray_pix) ray_pix[q] = pix;
+            if (pix >= 0) {
+                ++in_map;
+                if (count) {
+#pragma omp atomic
+                    count[pix] += 1;
+                }
+            } else if (pix == -1) {
+                ++outside;
+            } else {
+                ++lost;
+            }
+        }
+    }
+    if (stats) {
+        stats->rays_total = ni * nj;
+        stats->rays_in_map = in_map;
+        stats->rays_outside = outside;
+        stats->rays_lost = lost;
+    }
+    return 0;
+}
+
+// A list of individual lattice rays (ray_ij[2q] = i, ray_ij[2q+1] = j): sampled checks at the full-size configs.
+int oracle_shoot_rays(double kappa, double gamma, double s, double L, int npix, double d, const float* lens_xy,
+                      const float* lens_m, long long n_lens, const long long* ray_ij, long long n_rays, double* ray_y,
+                      double* ray_alpha, double* ray_scale, int* ray_pix, int n_threads) {
+    oracle_geometry g;
+    if (oracle_derive_geometry(kappa, gamma, s, L, npix, d, &g) != 0) return -1;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 64)
+    for (long long q = 0; q < n_rays; ++q) {
+        const double x1 = ((double)ray_ij[2 * q] + 0.5 - (double)g.n1 / 2.0) * d;
+        const double x2 = ((double)ray_ij[2 * q + 1] + 0.5 - (double)g.n2 / 2.0) * d;
+        double y1, y2, al1, al2, sc = 0.0;
+        shoot_one(x1, x2, g.kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, ray_scale ? &sc : nullptr);
+        if (ray_y) { ray_y[2 * q] = y1; ray_y[2 * q + 1] = y2; }
+        if (ray_alpha) { ray_alpha[2 * q] = al1; ray_alpha[2 * q + 1] = al2; }
+        if (ray_scale) ray_scale[q] = sc;
+        if (ray_pix) ray_pix[q] = pixel_of(y1, y2, L, g.p, npix);
+    }
+    return 0;
+}
+
+// Arbitrary image-plane positions (not lattice rays): used by pin P3 (hand sums, Appendix D of SURVEY.md).
+int oracle_map_points(double kappa, double gamma, double s, const float* lens_xy, const float* lens_m,
+                      long long n_lens, const double* x, long long n_pts, double* y, double* alpha) {
+    const double kappa_s = s * kappa;
+    for (long long q = 0; q < n_pts; ++q) {
+        double y1, y2, al1, al2;
+        shoot_one(x[2 * q], x[2 * q + 1], kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, nullptr);
+        y[2 * q] = y1; y[2 * q + 1] = y2;
+        if (alpha) { alpha[2 * q] = al1; alpha[2 * q + 1] = al2; }
+    }
+    return 0;
+}
+
+// Pixel ids for given source positions (exposes the S4 convention to the tests).
+void oracle_pixels_of(const double* y, long long n_pts, double L, int npix, int* pix) {
+    const double p = L / npix;
+    for (long long q = 0; q < n_pts; ++q) pix[q] = pixel_of(y[2 * q], y[2 * q + 1], L, p, npix);
+}
+
+// Eq. (4) with N_avg = (p/d)^2 (readings S5, S16).
+void oracle_magnification(const int* count, long long n_pixels, double n_avg, float* mag) {
+    for (long long q = 0; q < n_pixels; ++q) mag[q] = (float)((double)count[q] / n_avg);
+}
+
+int oracle_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+}  // extern "C"
