@@ -1,0 +1,125 @@
+/* mlens.h — C ABI of libmlens.so: direct inverse ray-shooting for quasar-microlensing magnification maps on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * The operation (Vernardos & Fluke 2014, arXiv:1406.0559; line numbers are of /root/reference/PAPER.md):
+ *   - PAPER.md:71   rays on a regular image-plane lattice are projected through the lens plane, "each deflected by
+ *                   N_* individual lenses ... and accumulated on a gridded source plane";
+ *   - PAPER.md:73   Eq. (1): y = diag(1-gamma, 1+gamma) x - kappa_s x - sum_{i=1..N_*} m_i (x - x_i)/|x - x_i|^2,
+ *                   summed DIRECTLY over all N_* point lenses for every ray (GPU-D);
+ *   - PAPER.md:75-77 Eq. (2): kappa = kappa_s + kappa_*, s = kappa_s/kappa;
+ *   - PAPER.md:85-87 Eq. (4): mu_ij = N_ij / N_avg;  here N_avg = (pixel/ray_spacing)^2 (BASELINE.json north_star);
+ *   - PAPER.md:294  the count map is 32-bit integers, Npix*Npix, row-major.
+ * Conventions the paper leaves open are listed in DESIGN.md ("Readings"): cell-centred symmetric lattice
+ * x = (i + 1/2 - n/2) d with n1 = 2*ceil(a1/d - 1e-9), a1 = 1.2 (L/2)/|1-kappa-gamma| (a2, n2 with +gamma);
+ * half-open pixels with floor, ix from y1, iy from y2, pixel id = iy*Npix + ix, corner of pixel (0,0) at
+ * (-L/2, -L/2); no softening — a ray with a non-finite source position is counted as "lost" and not binned.
+ *
+ * All lengths are in Einstein radii of the mean lens mass, masses in units of the mean mass.
+ *
+ * Every function returns MLENS_OK (0) or a negative mlens_status; none throws or aborts.  After a failure
+ * mlens_last_error() returns a thread-local description.  There is NO CPU fallback: without a CUDA device
+ * mlens_create fails with MLENS_ECUDA.  Pointers are marked HOST or DEVICE; DEVICE pointers must belong to the device
+ * that was current when mlens_create was called.  `cuda_stream` is a cudaStream_t passed as void* (NULL = the
+ * legacy default stream).  Calls on one handle must not be issued concurrently from several host threads.
+ */
+#ifndef MLENS_H_
+#define MLENS_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mlens mlens_t; /* opaque; owns the device copy of the lens list, device counters, scratch */
+
+typedef enum {
+    MLENS_OK = 0,
+    MLENS_EINVAL = -1, /* bad argument (see each function) */
+    MLENS_ENOMEM = -2, /* host or device allocation failed */
+    MLENS_ECUDA = -3,  /* CUDA runtime error (no device, launch failure, ...) */
+    MLENS_ERANGE = -4  /* lattice or map too large for the index types */
+} mlens_status;
+
+typedef struct {
+    long long rays_total;   /* rays shot since the counters were last reset */
+    long long rays_in_map;  /* rays binned into the count map */
+    long long rays_outside; /* finite source position outside the map */
+    long long rays_lost;    /* non-finite source position (ray exactly on a lens) */
+    long long n_lens;
+    int max_count;          /* largest pixel count seen by the last mlens_shoot / mlens_magnification (overflow guard,
+                               PAPER.md:692-698: the paper's largest observed count is 998 878) */
+    float elapsed_ms;       /* device time of the last mlens_shoot that was given a stats pointer, else 0 */
+} mlens_stats;
+
+typedef struct {
+    long long n1, n2;                  /* lattice ray counts along x1, x2 */
+    double a1, a2;                     /* shooting-rectangle half-widths */
+    double p, d;                       /* pixel size L/Npix, ray spacing */
+    double kappa_s, kappa_star, n_avg; /* Eq. 2 split; N_avg = (p/d)^2 */
+} mlens_geometry;
+
+/* Create a map context (a map is defined by kappa, gamma, s, width, resolution, N_avg and the
+ * lens positions/masses).
+ *   kappa, gamma, s    total convergence, shear, smooth-matter fraction (0 <= s <= 1)
+ *   map_side, npix     L > 0 and Npix > 0: side of the square source-plane map and its pixel count per side
+ *   ray_spacing        d > 0: image-plane lattice spacing
+ *   lens_xy            HOST, 2*n_lens floats, interleaved x,y; copied — the caller keeps ownership
+ *   lens_m             HOST, n_lens floats (> 0, finite), or NULL for m_i = 1
+ *   n_lens             >= 0 (0 = macro-model only)
+ * The lattice (n1, n2) and the rectangle are derived here (see mlens_get_geometry).
+ * Errors: MLENS_EINVAL for non-finite or out-of-range parameters, |1-kappa-gamma| or |1-kappa+gamma| < 1e-6 (critical
+ * line: the rectangle is unbounded), kappa < 0, NULL out / lens_xy (when n_lens > 0), a non-finite lens coordinate or a
+ * mass that is not finite and > 0;  MLENS_ERANGE if n1 or n2 >= 2^31 or npix^2 >= 2^31;  MLENS_ECUDA / MLENS_ENOMEM. */
+int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map_side, int npix, double ray_spacing,
+                 const float* lens_xy, const float* lens_m, long long n_lens);
+
+/* Shoot the whole lattice (steps a1-a5 of the hot path): zero `count_dev` and the ray counters, shoot all n1*n2
+ * rays, bin them, then — if `mag_dev` is not NULL — write mag = (float)((double)count / N_avg).
+ *   count_dev   DEVICE, npix*npix int32, row-major [iy][ix], caller-owned
+ *   mag_dev     DEVICE, npix*npix float32, or NULL
+ *   stats       HOST or NULL.  NULL: all work is only enqueued on `cuda_stream` and the call returns at once.
+ *               Non-NULL: the call synchronises the stream and fills *stats (elapsed_ms = device time of this call). */
+int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, mlens_stats* stats);
+
+/* Verification / partial shooting: rays i0 <= i < i0+ni, j0 <= j < j0+nj of the SAME lattice, through the SAME
+ * kernel.  ACCUMULATES into count_dev and into the ray counters (zero them yourself / mlens_reset_stats).
+ *   count_dev   DEVICE npix*npix int32, or NULL (no binning)
+ *   ray_y_dev   DEVICE ni*nj*2 doubles or NULL: source position of ray (ii, jj) at [2*(jj*ni+ii)], [.. + 1]
+ *   ray_pix_dev DEVICE ni*nj int32 or NULL: pixel id, -1 = outside the map, -2 = non-finite
+ * Asynchronous on `cuda_stream`.  MLENS_EINVAL if the block is not inside [0,n1) x [0,n2). */
+int mlens_shoot_block(mlens_t* h, long long i0, long long j0, long long ni, long long nj, int* count_dev,
+                      double* ray_y_dev, int* ray_pix_dev, void* cuda_stream);
+
+/* End-to-end convenience with HOST buffers: device buffers owned by the handle, mlens_shoot, copies back,
+ * synchronises.  count_host: HOST npix*npix int32; mag_host: HOST npix*npix float32 or NULL; stats: HOST or NULL. */
+int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* stats);
+
+/* Step a5 alone (Eq. 4): mag = (float)((double)count / N_avg); also refreshes max_count.  Asynchronous. */
+int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* cuda_stream);
+
+/* Derived lattice and parameters (pure host data; valid from mlens_create on). */
+int mlens_get_geometry(const mlens_t* h, mlens_geometry* g);
+
+/* Synchronise `cuda_stream` and read the device ray counters. */
+int mlens_get_stats(mlens_t* h, void* cuda_stream, mlens_stats* stats);
+
+/* Zero the device ray counters (asynchronous). */
+int mlens_reset_stats(mlens_t* h, void* cuda_stream);
+
+/* Tuning / ablation switches.  Keys:
+ *   "kernel"    0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 1 = FP32 difference-form kernel (default)
+ *   "binning"   0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
+ *               3 = + CTA-private shared-memory window
+ *   "ctas_per_sm"  persistent CTAs per SM (default 2)
+ * Returns MLENS_EINVAL for an unknown key or value. */
+int mlens_set_option(mlens_t* h, const char* key, long long value);
+
+/* Thread-local message for the last failure on this thread ("" if none). */
+const char* mlens_last_error(void);
+
+/* Frees everything mlens_create allocated (never the caller's buffers).  NULL is allowed. */
+void mlens_destroy(mlens_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLENS_H_ */

@@ -1,0 +1,323 @@
+// mlens.cu — host side of libmlens.so: the C ABI declared in include/mlens.h.
+// Argument checking, the derived lattice (DESIGN.md "Readings" S2), the device copy of the lens list, kernel launches.
+// No torch types, no CPU fallback: every step of the hot path runs in the kernels of shoot_kernel.cuh.
+#include "../../include/mlens.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "shoot_kernel.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define MLENS_CUDA(call)                                                                              \
+    do {                                                                                              \
+        cudaError_t e_ = (call);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail(e_ == cudaErrorMemoryAllocation ? MLENS_ENOMEM : MLENS_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                      \
+    } while (0)
+
+constexpr int kChunkMax = 2048;        // lenses per chunk when the list is streamed in several chunks
+constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chunk
+
+}  // namespace
+
+struct mlens {
+    // parameters
+    double kappa, gamma, s, L, d;
+    int npix;
+    long long n_lens;
+    mlens_geometry geo;
+    // device state
+    int device;
+    int sm_count;
+    float4* lens_dev;                  // (x, y, m, 0)
+    unsigned long long* counters_dev;  // in_map, outside, lost, total
+    int* max_count_dev;
+    unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
+    // host-buffer path
+    int* count_own;
+    float* mag_own;
+    cudaStream_t own_stream;
+    cudaEvent_t ev0, ev1;
+    float last_ms;
+    // options
+    int opt_kernel, opt_binning, opt_ctas_per_sm;
+};
+
+namespace {
+
+int check_handle(const mlens_t* h) { return h ? MLENS_OK : fail(MLENS_EINVAL, "NULL handle"); }
+
+int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long nj, int* count, double* ray_y,
+                 int* ray_pix, cudaStream_t st) {
+    if (ni == 0 || nj == 0) return MLENS_OK;
+    mlk::ShootParams P;
+    memset(&P, 0, sizeof(P));
+    P.i0 = i0; P.j0 = j0; P.ni = ni; P.nj = nj;
+    P.half_n1 = (double)h->geo.n1 / 2.0;
+    P.half_n2 = (double)h->geo.n2 / 2.0;
+    P.d = h->d;
+    P.tiles_x = (int)((ni + mlk::kTile - 1) / mlk::kTile);
+    P.tiles_y = (int)((nj + mlk::kTile - 1) / mlk::kTile);
+    P.f1 = 1.0 - h->geo.kappa_s - h->gamma;
+    P.f2 = 1.0 - h->geo.kappa_s + h->gamma;
+    P.half_L = h->L / 2.0;
+    P.p = h->geo.p;
+    P.npix = h->npix;
+    P.lens_raw = h->lens_dev;
+    P.n_lens = (int)h->n_lens;
+    P.rho2 = 0.25;  // rho = 0.5 sqrt(max(m,1))
+    P.count = count; P.ray_y = ray_y; P.ray_pix = ray_pix;
+    P.counters = h->counters_dev;
+    P.bin_mode = h->opt_binning;
+
+    if (h->opt_kernel == 0) {
+        const long long n_rays = ni * nj;
+        long long blocks = (n_rays + 255) / 256;
+        const long long cap = (long long)h->sm_count * 16;
+        if (blocks > cap) blocks = cap;
+        mlk::shoot_fp64_kernel<<<(unsigned)blocks, 256, 0, st>>>(P);
+        MLENS_CUDA(cudaGetLastError());
+        return MLENS_OK;
+    }
+
+    int chunk, n_chunks;
+    if (P.n_lens <= kChunkSingleMax) {
+        chunk = (P.n_lens + 3) & ~3;
+        if (chunk < 4) chunk = 4;
+        n_chunks = 1;
+    } else {
+        chunk = kChunkMax;
+        n_chunks = (P.n_lens + chunk - 1) / chunk;
+    }
+    P.chunk = chunk; P.n_chunks = n_chunks;
+    const size_t smem = sizeof(mlk::TileShared) + (size_t)chunk * 16 * (n_chunks > 1 ? 3 : 2);
+    MLENS_CUDA(cudaFuncSetAttribute(mlk::shoot_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
+    long long grid = (long long)h->sm_count * h->opt_ctas_per_sm;
+    if (grid > n_tiles) grid = n_tiles;
+    mlk::shoot_fp32_kernel<<<(unsigned)grid, mlk::kThreads, smem, st>>>(P);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int launch_magnification(mlens_t* h, const int* count, float* mag, cudaStream_t st) {
+    const long long n = (long long)h->npix * h->npix;
+    MLENS_CUDA(cudaMemsetAsync(h->max_count_dev, 0, sizeof(int), st));
+    long long blocks = (n / 4 + 255) / 256;
+    const long long cap = (long long)h->sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    mlk::magnification_kernel<<<(unsigned)blocks, 256, 0, st>>>(count, mag, n, h->geo.n_avg, h->max_count_dev);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int read_stats(mlens_t* h, cudaStream_t st, mlens_stats* out) {
+    MLENS_CUDA(cudaMemcpyAsync(h->counters_host, h->counters_dev, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 4, h->max_count_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    MLENS_CUDA(cudaStreamSynchronize(st));
+    out->rays_in_map = (long long)h->counters_host[0];
+    out->rays_outside = (long long)h->counters_host[1];
+    out->rays_lost = (long long)h->counters_host[2];
+    out->rays_total = (long long)h->counters_host[3];
+    out->n_lens = h->n_lens;
+    int mc;
+    memcpy(&mc, h->counters_host + 4, sizeof(int));
+    out->max_count = mc;
+    out->elapsed_ms = h->last_ms;
+    return MLENS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mlens_last_error(void) { return g_err; }
+
+int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map_side, int npix, double ray_spacing,
+                 const float* lens_xy, const float* lens_m, long long n_lens) {
+    if (!out) return fail(MLENS_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!std::isfinite(kappa) || !std::isfinite(gamma) || !std::isfinite(s) || !std::isfinite(map_side) ||
+        !std::isfinite(ray_spacing))
+        return fail(MLENS_EINVAL, "non-finite parameter");
+    if (kappa < 0) return fail(MLENS_EINVAL, "kappa < 0");
+    if (s < 0 || s > 1) return fail(MLENS_EINVAL, "s outside [0,1]");
+    if (!(map_side > 0) || npix <= 0 || !(ray_spacing > 0)) return fail(MLENS_EINVAL, "map_side, npix, ray_spacing must be > 0");
+    if (n_lens < 0) return fail(MLENS_EINVAL, "n_lens < 0");
+    if (n_lens > 0 && !lens_xy) return fail(MLENS_EINVAL, "lens_xy is NULL");
+    if (n_lens > (1ll << 30)) return fail(MLENS_ERANGE, "n_lens too large");
+    const double f1 = std::fabs(1.0 - kappa - gamma), f2 = std::fabs(1.0 - kappa + gamma);
+    if (f1 < 1e-6 || f2 < 1e-6) return fail(MLENS_EINVAL, "macro-model on the critical line: |1-kappa-+gamma| < 1e-6");
+    if ((long long)npix * npix >= (1ll << 31)) return fail(MLENS_ERANGE, "npix^2 >= 2^31");
+
+    mlens_geometry g;
+    g.kappa_s = s * kappa;
+    g.kappa_star = kappa - g.kappa_s;
+    g.p = map_side / npix;
+    g.d = ray_spacing;
+    g.a1 = 1.2 * (map_side / 2.0) / f1;
+    g.a2 = 1.2 * (map_side / 2.0) / f2;
+    const double c1 = std::ceil(g.a1 / ray_spacing - 1e-9), c2 = std::ceil(g.a2 / ray_spacing - 1e-9);
+    if (!(c1 < 1073741824.0) || !(c2 < 1073741824.0)) return fail(MLENS_ERANGE, "lattice has >= 2^31 rays along an axis");
+    g.n1 = 2 * (long long)c1;
+    g.n2 = 2 * (long long)c2;
+    g.n_avg = (g.p / ray_spacing) * (g.p / ray_spacing);
+
+    std::vector<float4> packed((size_t)n_lens);
+    for (long long k = 0; k < n_lens; ++k) {
+        const float x = lens_xy[2 * k], y = lens_xy[2 * k + 1], m = lens_m ? lens_m[k] : 1.0f;
+        if (!std::isfinite(x) || !std::isfinite(y)) return fail(MLENS_EINVAL, "lens %lld has a non-finite coordinate", k);
+        if (!std::isfinite(m) || !(m > 0)) return fail(MLENS_EINVAL, "lens %lld has a mass that is not finite and > 0", k);
+        packed[(size_t)k] = make_float4(x, y, m, 0.f);
+    }
+
+    int dev = 0;
+    MLENS_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    MLENS_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major < 10) return fail(MLENS_ECUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
+
+    mlens* h = new (std::nothrow) mlens();
+    if (!h) return fail(MLENS_ENOMEM, "host allocation failed");
+    memset(h, 0, sizeof(*h));
+    h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
+    h->npix = npix; h->n_lens = n_lens; h->geo = g;
+    h->device = dev; h->sm_count = prop.multiProcessorCount;
+    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2;
+
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
+    if (e == cudaSuccess && n_lens > 0)
+        e = cudaMemcpy(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&h->counters_dev, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&h->max_count_dev, sizeof(int));
+    if (e == cudaSuccess) e = cudaMemset(h->max_count_dev, 0, sizeof(int));
+    if (e == cudaSuccess) e = cudaMallocHost(&h->counters_host, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaEventCreate(&h->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&h->ev1);
+    if (e != cudaSuccess) {
+        const int code = fail(e == cudaErrorMemoryAllocation ? MLENS_ENOMEM : MLENS_ECUDA, "mlens_create: %s", cudaGetErrorString(e));
+        mlens_destroy(h);
+        return code;
+    }
+    *out = h;
+    return MLENS_OK;
+}
+
+void mlens_destroy(mlens_t* h) {
+    if (!h) return;
+    if (h->lens_dev) cudaFree(h->lens_dev);
+    if (h->counters_dev) cudaFree(h->counters_dev);
+    if (h->max_count_dev) cudaFree(h->max_count_dev);
+    if (h->counters_host) cudaFreeHost(h->counters_host);
+    if (h->count_own) cudaFree(h->count_own);
+    if (h->mag_own) cudaFree(h->mag_own);
+    if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    if (h->ev0) cudaEventDestroy(h->ev0);
+    if (h->ev1) cudaEventDestroy(h->ev1);
+    delete h;
+}
+
+int mlens_get_geometry(const mlens_t* h, mlens_geometry* g) {
+    if (!h || !g) return fail(MLENS_EINVAL, "NULL argument");
+    *g = h->geo;
+    return MLENS_OK;
+}
+
+int mlens_set_option(mlens_t* h, const char* key, long long value) {
+    if (!h || !key) return fail(MLENS_EINVAL, "NULL argument");
+    if (!strcmp(key, "kernel")) {
+        if (value < 0 || value > 1) return fail(MLENS_EINVAL, "kernel must be 0 or 1");
+        h->opt_kernel = (int)value;
+    } else if (!strcmp(key, "binning")) {
+        if (value < 0 || value > 3) return fail(MLENS_EINVAL, "binning must be 0..3");
+        h->opt_binning = (int)value;
+    } else if (!strcmp(key, "ctas_per_sm")) {
+        if (value < 1 || value > 8) return fail(MLENS_EINVAL, "ctas_per_sm must be 1..8");
+        h->opt_ctas_per_sm = (int)value;
+    } else {
+        return fail(MLENS_EINVAL, "unknown option '%s'", key);
+    }
+    return MLENS_OK;
+}
+
+int mlens_reset_stats(mlens_t* h, void* cuda_stream) {
+    if (int rc = check_handle(h)) return rc;
+    MLENS_CUDA(cudaMemsetAsync(h->counters_dev, 0, 4 * sizeof(unsigned long long), (cudaStream_t)cuda_stream));
+    return MLENS_OK;
+}
+
+int mlens_get_stats(mlens_t* h, void* cuda_stream, mlens_stats* stats) {
+    if (!h || !stats) return fail(MLENS_EINVAL, "NULL argument");
+    return read_stats(h, (cudaStream_t)cuda_stream, stats);
+}
+
+int mlens_shoot_block(mlens_t* h, long long i0, long long j0, long long ni, long long nj, int* count_dev,
+                      double* ray_y_dev, int* ray_pix_dev, void* cuda_stream) {
+    if (int rc = check_handle(h)) return rc;
+    if (i0 < 0 || j0 < 0 || ni < 0 || nj < 0 || i0 + ni > h->geo.n1 || j0 + nj > h->geo.n2)
+        return fail(MLENS_EINVAL, "block [%lld,+%lld) x [%lld,+%lld) is outside the %lld x %lld lattice", i0, ni, j0, nj,
+                    h->geo.n1, h->geo.n2);
+    return launch_block(h, i0, j0, ni, nj, count_dev, ray_y_dev, ray_pix_dev, (cudaStream_t)cuda_stream);
+}
+
+int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* cuda_stream) {
+    if (!h || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    return launch_magnification(h, count_dev, mag_dev, (cudaStream_t)cuda_stream);
+}
+
+int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, mlens_stats* stats) {
+    if (!h || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t n = (size_t)h->npix * h->npix;
+    if (stats) MLENS_CUDA(cudaEventRecord(h->ev0, st));
+    MLENS_CUDA(cudaMemsetAsync(count_dev, 0, n * sizeof(int), st));
+    MLENS_CUDA(cudaMemsetAsync(h->counters_dev, 0, 4 * sizeof(unsigned long long), st));
+    if (int rc = launch_block(h, 0, 0, h->geo.n1, h->geo.n2, count_dev, nullptr, nullptr, st)) return rc;
+    if (int rc = launch_magnification(h, count_dev, mag_dev, st)) return rc;
+    if (stats) {
+        MLENS_CUDA(cudaEventRecord(h->ev1, st));
+        MLENS_CUDA(cudaEventSynchronize(h->ev1));
+        MLENS_CUDA(cudaEventElapsedTime(&h->last_ms, h->ev0, h->ev1));
+        return read_stats(h, st, stats);
+    }
+    return MLENS_OK;
+}
+
+int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* stats) {
+    if (!h || !count_host) return fail(MLENS_EINVAL, "NULL argument");
+    const size_t n = (size_t)h->npix * h->npix;
+    if (!h->own_stream) MLENS_CUDA(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
+    if (!h->count_own) MLENS_CUDA(cudaMalloc(&h->count_own, n * sizeof(int)));
+    if (mag_host && !h->mag_own) MLENS_CUDA(cudaMalloc(&h->mag_own, n * sizeof(float)));
+    mlens_stats local;
+    if (int rc = mlens_shoot(h, h->count_own, mag_host ? h->mag_own : nullptr, h->own_stream, &local)) return rc;
+    MLENS_CUDA(cudaMemcpyAsync(count_host, h->count_own, n * sizeof(int), cudaMemcpyDeviceToHost, h->own_stream));
+    if (mag_host) MLENS_CUDA(cudaMemcpyAsync(mag_host, h->mag_own, n * sizeof(float), cudaMemcpyDeviceToHost, h->own_stream));
+    MLENS_CUDA(cudaStreamSynchronize(h->own_stream));
+    if (stats) *stats = local;
+    return MLENS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,444 @@
+// shoot_kernel.cuh — sm_100a device code of libmlens.so.
+//
+// shoot_fp32_kernel: the production kernel.  Persistent CTAs walk 64x64-ray tiles of the image-plane lattice
+// (Fig. 1).  For every ray the deflection of Eq. (1) is summed DIRECTLY over all N_*
+// lenses, in the algebraically identical "difference form" that keeps FP32 rounding harmless:
+//
+//   z = x1 + i x2,  conj(alpha)(z) = sum_i m_i/(z - z_i).   With the tile centre Z_c (FP64), zeta_i = Z_c - z_i,
+//   delta = z - Z_c and c_i = m_i/zeta_i:
+//       m_i/(zeta_i + delta) = c_i - delta * c_i/(zeta_i + delta)
+//   =>  conj(alpha) = A_c - delta * S(delta),   A_c = sum_i c_i (FP64, once per tile),
+//                                               S   = sum_i c_i conj(w_i)/|w_i|^2,  w_i = zeta_i + delta  (FP32 loop)
+//
+// Per interaction: 1 packed FADD2 + 5 packed FFMA2 per PAIR of rays and one MUFU.RCP per ray.  Lenses within rho of
+// the tile centre are summed per ray in plain FP64 instead (near list).  The per-ray epilogue (Eq. 1 macro term,
+// pixel id) is FP64; binning ("accumulated on a gridded source plane") uses integer REDs, so the map does
+// not depend on the order of execution.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mlk {
+
+constexpr int kThreads = 256;       // threads per CTA
+constexpr int kTile = 64;           // tile is kTile x kTile rays
+constexpr int kR = 16;              // rays per thread, consecutive along x1
+constexpr int kNearMax = 32;        // capacity of the per-tile near-lens list
+constexpr int kWin = 32;            // binning window side (pixels), BIN_WINDOW mode
+constexpr float kFar = 1.0e15f;     // offset of a neutralised main-list entry (contributes exactly 0)
+
+enum BinMode { BIN_PER_RAY = 0, BIN_RUNS = 1, BIN_WARP = 2, BIN_WINDOW = 3 };
+
+struct ShootParams {
+    // lattice and block
+    long long i0, j0, ni, nj;       // block of rays to shoot
+    double half_n1, half_n2;        // n1/2, n2/2
+    double d;                       // ray spacing
+    int tiles_x, tiles_y;
+    // macro model and map
+    double f1, f2;                  // 1-kappa_s-gamma, 1-kappa_s+gamma
+    double half_L, p;               // L/2, pixel size
+    int npix;
+    // lenses
+    const float4* lens_raw;         // (x, y, m, 0) per lens, global memory
+    int n_lens;
+    int chunk;                      // lenses per shared-memory chunk (multiple of 4)
+    int n_chunks;
+    double rho2;                    // near-list radius^2 for m <= 1 (scaled by max(m,1))
+    // outputs
+    int* count;                     // npix*npix or nullptr
+    double* ray_y;                  // optional per-ray outputs
+    int* ray_pix;
+    unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total
+    int bin_mode;
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D bulk copy (TMA engine, SASS UBLKCP), MUFU reciprocal
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ float rcp_mufu(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// binning helpers (step a4)
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void red_add(int* addr, int v) { atomicAdd(addr, v); }  // result unused -> RED.E.ADD
+
+// warp-aggregated add: lanes holding the same pixel elect a leader that adds the group's total once
+__device__ __forceinline__ void warp_aggregated_add(int* count, int pix, int n, bool active) {
+    const unsigned lane = threadIdx.x & 31;
+    unsigned live = __ballot_sync(0xffffffffu, active);
+    if (!active) return;
+    unsigned peers = __match_any_sync(live, pix);
+    int leader = __ffs(peers) - 1;
+    const int total = __reduce_add_sync(peers, n);
+    if ((int)lane == leader) red_add(count + pix, total);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// the production kernel
+// ---------------------------------------------------------------------------------------------------------------
+struct __align__(16) TileShared {
+    uint64_t bar[2];                         // mbarriers of the raw-chunk double buffer
+    double part[kThreads / 32][2];           // per-warp partial sums of A_c
+    double near_zx[kNearMax], near_zy[kNearMax], near_m[kNearMax];
+    int near_n;
+    int win_ix0, win_iy0;                    // binning window origin (BIN_WINDOW)
+    unsigned long long ctr[3];               // CTA-private ray counters
+    int win[kWin * kWin];                    // CTA-private count window (BIN_WINDOW)
+};
+
+// a finished run (pix, n) of one thread goes to the map by the selected route; called convergently by the whole warp
+__device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, int pix, int n, bool active) {
+    if (P.bin_mode == BIN_WARP) {
+        warp_aggregated_add(P.count, pix, n, active);
+    } else if (active) {
+        if (P.bin_mode == BIN_RUNS) {
+            red_add(P.count + pix, n);
+        } else {  // BIN_WINDOW: CTA-private shared-memory window, global RED for strays
+            const int wx = pix % P.npix - sh.win_ix0, wy = pix / P.npix - sh.win_iy0;
+            if ((unsigned)wx < (unsigned)kWin && (unsigned)wy < (unsigned)kWin)
+                atomicAdd(&sh.win[wy * kWin + wx], n);
+            else
+                red_add(P.count + pix, n);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
+    TileShared& sh = *reinterpret_cast<TileShared*>(smem_raw_bytes);
+    float4* xf = reinterpret_cast<float4*>(smem_raw_bytes + sizeof(TileShared));  // transformed chunk
+    float4* raw0 = xf + P.chunk;                                                   // raw staging buffer(s)
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int tx = tid & 3, ty = tid >> 2;  // 4 threads x 16 rays along x1, 64 rows along x2
+
+    if (tid == 0) {
+        mbar_init(&sh.bar[0], 1);
+        mbar_init(&sh.bar[1], 1);
+        mbar_fence_init();
+        sh.ctr[0] = sh.ctr[1] = sh.ctr[2] = 0ull;
+        sh.near_n = 0;
+    }
+    __syncthreads();
+
+    // in-tile offsets delta (FP32), identical for every tile
+    const float dyf = (float)(((double)ty - 31.5) * P.d);
+    float2 dxb[kR / 2];
+#pragma unroll
+    for (int j = 0; j < kR / 2; ++j) {
+        dxb[j].x = (float)(((double)(tx * kR + 2 * j) - 31.5) * P.d);
+        dxb[j].y = (float)(((double)(tx * kR + 2 * j + 1) - 31.5) * P.d);
+    }
+
+    const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
+    long long g = 0;  // sequence number of the raw-chunk load being consumed: buffer g&1, barrier phase (g>>1)&1
+
+    // single-chunk case: the raw list is staged once and reused by every tile
+    if (P.n_lens > 0 && tid == 0 && blockIdx.x < n_tiles) {
+        const uint32_t bytes = (uint32_t)min(P.chunk, P.n_lens) * 16u;
+        mbar_arrive_expect_tx(&sh.bar[0], bytes);
+        bulk_copy_g2s(raw0, P.lens_raw, bytes, &sh.bar[0]);
+    }
+
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
+        const long long ti0 = P.i0 + (long long)tI * kTile, tj0 = P.j0 + (long long)tJ * kTile;
+        const double Zcx = ((double)(ti0 + kTile / 2) - P.half_n1) * P.d;
+        const double Zcy = ((double)(tj0 + kTile / 2) - P.half_n2) * P.d;
+
+        float2 Sr[kR / 2], Si[kR / 2];
+#pragma unroll
+        for (int j = 0; j < kR / 2; ++j) Sr[j] = Si[j] = make_float2(0.f, 0.f);
+        double Acr = 0.0, Aci = 0.0;
+
+        for (int c = 0; c < P.n_chunks && P.n_lens > 0; ++c) {
+            const int l0 = c * P.chunk;
+            const int n_c = min(P.chunk, P.n_lens - l0);
+            const int buf = (int)(g & 1);
+            float4* raw = raw0 + (size_t)buf * P.chunk;
+            // (1) raw chunk landed?  (single-chunk lists are staged once and stay resident: only load 0 is waited for)
+            if (P.n_chunks > 1 || tile == (long long)blockIdx.x) mbar_wait(&sh.bar[buf], (uint32_t)((g >> 1) & 1));
+            // (2) per-tile FP64 transform: zeta = Z_c - z_i, c = m/zeta; near lenses go to the FP64 list
+            double pr_ = 0.0, pi_ = 0.0;
+            const int n_pad = (n_c + 3) & ~3;
+            for (int t = tid; t < n_pad; t += kThreads) {
+                float4 o = make_float4(kFar, kFar, 0.f, 0.f);
+                if (t < n_c) {
+                    const float4 q = raw[t];
+                    const double zx = Zcx - (double)q.x, zy = Zcy - (double)q.y, m = (double)q.z;
+                    const double r2 = zx * zx + zy * zy;
+                    bool near = r2 < P.rho2 * fmax(m, 1.0);
+                    if (near) {
+                        const int slot = atomicAdd(&sh.near_n, 1);
+                        if (slot < kNearMax) {
+                            sh.near_zx[slot] = zx; sh.near_zy[slot] = zy; sh.near_m[slot] = m;
+                        } else {
+                            near = false;  // list full: keep the lens in the FP32 list (still summed, less accurate)
+                        }
+                    }
+                    if (!near) {
+                        const double inv = m / r2;
+                        const double cr = zx * inv, ci = -zy * inv;
+                        pr_ += cr; pi_ += ci;
+                        o = make_float4((float)zx, (float)zy, (float)cr, (float)ci);
+                    }
+                }
+                xf[t] = o;
+            }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                pr_ += __shfl_xor_sync(0xffffffffu, pr_, off);
+                pi_ += __shfl_xor_sync(0xffffffffu, pi_, off);
+            }
+            if (lane == 0) { sh.part[warp][0] = pr_; sh.part[warp][1] = pi_; }
+            __syncthreads();
+            // (3) prefetch the next raw chunk (multi-chunk only): the buffer it overwrites was consumed one chunk ago
+            if (P.n_chunks > 1 && tid == 0) {
+                int cn = c + 1;
+                long long tn = tile;
+                if (cn == P.n_chunks) { cn = 0; tn = tile + gridDim.x; }
+                if (tn < n_tiles) {
+                    const int nb = (int)((g + 1) & 1);
+                    const uint32_t bytes = (uint32_t)min(P.chunk, P.n_lens - cn * P.chunk) * 16u;
+                    mbar_arrive_expect_tx(&sh.bar[nb], bytes);
+                    bulk_copy_g2s(raw0 + (size_t)nb * P.chunk, P.lens_raw + (size_t)cn * P.chunk, bytes, &sh.bar[nb]);
+                }
+            }
+            if (P.n_chunks > 1) ++g;
+#pragma unroll
+            for (int w = 0; w < kThreads / 32; ++w) { Acr += sh.part[w][0]; Aci += sh.part[w][1]; }
+
+            // (4) HOT LOOP: all lenses of the chunk x this thread's kR rays
+#pragma unroll 2
+            for (int l = 0; l < n_pad; ++l) {
+                const float4 q = xf[l];  // broadcast LDS.128: (zeta_x, zeta_y, c_r, c_i)
+                const float dy = dyf + q.y;
+                const float dy2 = dy * dy;
+                const float a = q.w * dy;    //  c_i * dy
+                const float b = -q.z * dy;   // -c_r * dy
+                const float2 NX = make_float2(q.x, q.x), DY2 = make_float2(dy2, dy2);
+                const float2 AA = make_float2(a, a), BB = make_float2(b, b);
+                const float2 CR = make_float2(q.z, q.z), CI = make_float2(q.w, q.w);
+#pragma unroll
+                for (int j = 0; j < kR / 2; ++j) {
+                    const float2 dx = __fadd2_rn(dxb[j], NX);
+                    const float2 r2 = __ffma2_rn(dx, dx, DY2);
+                    const float2 rc = make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y));
+                    const float2 pr = __ffma2_rn(CR, dx, AA);
+                    const float2 pi = __ffma2_rn(CI, dx, BB);
+                    Sr[j] = __ffma2_rn(pr, rc, Sr[j]);
+                    Si[j] = __ffma2_rn(pi, rc, Si[j]);
+                }
+            }
+            __syncthreads();  // xf (and sh.part) may be overwritten by the next chunk / tile
+        }
+
+        // (5) per-ray FP64 epilogue: alpha, Eq. (1), pixel id; (6) binning
+        const int n_near = min(sh.near_n, kNearMax);
+        const long long jray = tj0 + ty;
+        const bool row_ok = jray < P.j0 + P.nj;
+        const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
+        const double dyd = (double)dyf;
+        int n_in = 0, n_out = 0, n_lost = 0;
+        int run_pix = -1, run_n = 0;
+
+        if (P.bin_mode == BIN_WINDOW) {
+            // window origin: pixel of the tile centre under the macro-model plus the tile-centre deflection
+            if (tid == 0) {
+                const double yc1 = P.f1 * Zcx - Acr, yc2 = P.f2 * Zcy + Aci;
+                const double u1 = (yc1 + P.half_L) / P.p, u2 = (yc2 + P.half_L) / P.p;
+                sh.win_ix0 = (u1 > -1e9 && u1 < 1e9) ? (int)floor(u1) - kWin / 2 : -(1 << 30);
+                sh.win_iy0 = (u2 > -1e9 && u2 < 1e9) ? (int)floor(u2) - kWin / 2 : -(1 << 30);
+            }
+            for (int t = tid; t < kWin * kWin; t += kThreads) sh.win[t] = 0;
+            __syncthreads();
+        }
+
+#pragma unroll
+        for (int k = 0; k < kR; ++k) {
+            const int j = k >> 1;
+            const float srf = (k & 1) ? Sr[j].y : Sr[j].x;
+            const float sif = (k & 1) ? Si[j].y : Si[j].x;
+            const float dxf = (k & 1) ? dxb[j].y : dxb[j].x;
+            const long long iray = ti0 + tx * kR + k;
+            const bool ok = row_ok && iray < P.i0 + P.ni;
+            const double dxd = (double)dxf, sr = (double)srf, si = (double)sif;
+            // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im)
+            double al1 = Acr - (dxd * sr - dyd * si);
+            double al2 = -(Aci - (dxd * si + dyd * sr));
+            for (int q = 0; q < n_near; ++q) {
+                const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyd;
+                const double f = sh.near_m[q] / (wx * wx + wy * wy);
+                al1 += f * wx;
+                al2 += f * wy;
+            }
+            const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
+            const double y1 = P.f1 * x1 - al1;
+            const double y2 = P.f2 * x2 - al2;
+            int pix;
+            if (!(isfinite(y1) && isfinite(y2))) {
+                pix = -2;
+            } else {
+                const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
+                if (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
+                    pix = (int)floor(u2) * P.npix + (int)floor(u1);
+                else
+                    pix = -1;
+            }
+            if (ok) {
+                n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
+                if (P.ray_y || P.ray_pix) {
+                    const long long qidx = (jray - P.j0) * P.ni + (iray - P.i0);
+                    if (P.ray_y) { P.ray_y[2 * qidx] = y1; P.ray_y[2 * qidx + 1] = y2; }
+                    if (P.ray_pix) P.ray_pix[qidx] = pix;
+                }
+            }
+            if (P.count) {
+                const int bp = ok ? pix : -1;
+                if (P.bin_mode == BIN_PER_RAY) {
+                    if (bp >= 0) red_add(P.count + bp, 1);
+                } else {
+                    // thread-local run-combine: consecutive rays of a thread mostly share a pixel
+                    const bool flush = (bp != run_pix);
+                    flush_run(P, sh, run_pix, run_n, flush && run_pix >= 0);
+                    if (flush) { run_pix = bp; run_n = 1; } else { ++run_n; }
+                }
+            }
+        }
+        if (P.count && P.bin_mode != BIN_PER_RAY) flush_run(P, sh, run_pix, run_n, run_pix >= 0);
+        n_in = __reduce_add_sync(0xffffffffu, n_in);
+        n_out = __reduce_add_sync(0xffffffffu, n_out);
+        n_lost = __reduce_add_sync(0xffffffffu, n_lost);
+        if (lane == 0) {
+            if (n_in) atomicAdd(&sh.ctr[0], (unsigned long long)n_in);
+            if (n_out) atomicAdd(&sh.ctr[1], (unsigned long long)n_out);
+            if (n_lost) atomicAdd(&sh.ctr[2], (unsigned long long)n_lost);
+        }
+        __syncthreads();  // all epilogues done: near list and window are complete
+        if (P.bin_mode == BIN_WINDOW && P.count) {
+            for (int t = tid; t < kWin * kWin; t += kThreads) {
+                const int v = sh.win[t];
+                if (v) {
+                    const int ix = sh.win_ix0 + (t % kWin), iy = sh.win_iy0 + (t / kWin);
+                    red_add(P.count + (size_t)iy * P.npix + ix, v);
+                }
+            }
+        }
+        if (tid == 0) sh.near_n = 0;
+        __syncthreads();
+    }
+
+    if (tid == 0) {
+        if (sh.ctr[0]) atomicAdd(&P.counters[0], sh.ctr[0]);
+        if (sh.ctr[1]) atomicAdd(&P.counters[1], sh.ctr[1]);
+        if (sh.ctr[2]) atomicAdd(&P.counters[2], sh.ctr[2]);
+        const unsigned long long tot = sh.ctr[0] + sh.ctr[1] + sh.ctr[2];
+        if (tot) atomicAdd(&P.counters[3], tot);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// plumbing / debug kernel: Eq. (1) in plain FP64, one ray per thread, lenses read from global memory
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) shoot_fp64_kernel(const ShootParams P) {
+    const long long n_rays = P.ni * P.nj;
+    int n_in = 0, n_out = 0, n_lost = 0;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n_rays; q += (long long)gridDim.x * blockDim.x) {
+        const long long jj = q / P.ni, ii = q - jj * P.ni;
+        const double x1 = ((double)(P.i0 + ii) + 0.5 - P.half_n1) * P.d;
+        const double x2 = ((double)(P.j0 + jj) + 0.5 - P.half_n2) * P.d;
+        double a1 = 0.0, a2 = 0.0;
+        for (int k = 0; k < P.n_lens; ++k) {
+            const float4 l = __ldg(P.lens_raw + k);
+            const double dx = x1 - (double)l.x, dy = x2 - (double)l.y;
+            const double w = (double)l.z / (dx * dx + dy * dy);
+            a1 += w * dx;
+            a2 += w * dy;
+        }
+        const double y1 = P.f1 * x1 - a1, y2 = P.f2 * x2 - a2;
+        int pix;
+        if (!(isfinite(y1) && isfinite(y2))) {
+            pix = -2;
+        } else {
+            const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
+            pix = (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
+                      ? (int)floor(u2) * P.npix + (int)floor(u1) : -1;
+        }
+        n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
+        if (P.ray_y) { P.ray_y[2 * q] = y1; P.ray_y[2 * q + 1] = y2; }
+        if (P.ray_pix) P.ray_pix[q] = pix;
+        if (P.count && pix >= 0) red_add(P.count + pix, 1);
+    }
+    n_in = __reduce_add_sync(0xffffffffu, n_in);
+    n_out = __reduce_add_sync(0xffffffffu, n_out);
+    n_lost = __reduce_add_sync(0xffffffffu, n_lost);
+    if ((threadIdx.x & 31) == 0) {
+        if (n_in) atomicAdd(&P.counters[0], (unsigned long long)n_in);
+        if (n_out) atomicAdd(&P.counters[1], (unsigned long long)n_out);
+        if (n_lost) atomicAdd(&P.counters[2], (unsigned long long)n_lost);
+        if (n_in + n_out + n_lost) atomicAdd(&P.counters[3], (unsigned long long)(n_in + n_out + n_lost));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// step a5 (Eq. 4): mag = (float)((double)count / N_avg); HBM-bound, 8 B per pixel
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) magnification_kernel(const int* __restrict__ count, float* __restrict__ mag,
+                                                            long long n, double n_avg, int* __restrict__ max_count) {
+    int vmax = 0;
+    const long long n4 = n >> 2;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += stride) {
+        const int4 c = __ldg(reinterpret_cast<const int4*>(count) + q);
+        vmax = max(max(vmax, max(c.x, c.y)), max(c.z, c.w));
+        if (mag) {
+            float4 m;
+            m.x = (float)((double)c.x / n_avg); m.y = (float)((double)c.y / n_avg);
+            m.z = (float)((double)c.z / n_avg); m.w = (float)((double)c.w / n_avg);
+            reinterpret_cast<float4*>(mag)[q] = m;
+        }
+    }
+    for (long long q = (n4 << 2) + (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
+        const int c = count[q];
+        vmax = max(vmax, c);
+        if (mag) mag[q] = (float)((double)c / n_avg);
+    }
+    vmax = __reduce_max_sync(0xffffffffu, vmax);
+    if ((threadIdx.x & 31) == 0 && vmax > 0) atomicMax(max_count, vmax);
+}
+
+}  // namespace mlk

@@ -1,0 +1,185 @@
+"""Thin ctypes binding of ``libmlens.so`` (``include/mlens.h``): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the hot path runs in the CUDA kernels behind the C ABI.
+There is no CPU fallback: if the library has not been built (``python -c "import __graft_entry__ as g; g.build()"``
+or ``python -m paper_1406_0559_b200.build``) or no CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "lib", "libmlens.so")
+_lib = None
+
+OK, EINVAL, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4
+
+
+class MlensError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"mlens error {code}: {msg}")
+        self.code = code
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [("rays_total", ctypes.c_longlong), ("rays_in_map", ctypes.c_longlong),
+                ("rays_outside", ctypes.c_longlong), ("rays_lost", ctypes.c_longlong), ("n_lens", ctypes.c_longlong),
+                ("max_count", ctypes.c_int), ("elapsed_ms", ctypes.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Geometry(ctypes.Structure):
+    _fields_ = [("n1", ctypes.c_longlong), ("n2", ctypes.c_longlong), ("a1", ctypes.c_double), ("a2", ctypes.c_double),
+                ("p", ctypes.c_double), ("d", ctypes.c_double), ("kappa_s", ctypes.c_double),
+                ("kappa_star", ctypes.c_double), ("n_avg", ctypes.c_double)]
+
+
+def lib() -> ctypes.CDLL:
+    """Load libmlens.so and declare the prototypes of every symbol in include/mlens.h.  Raises if it is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it first (__graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ll, dbl, ci = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_double, ctypes.c_int
+    L.mlens_create.argtypes = [ctypes.POINTER(vp), dbl, dbl, dbl, dbl, ci, dbl, vp, vp, ll]
+    L.mlens_shoot.argtypes = [vp, vp, vp, vp, ctypes.POINTER(Stats)]
+    L.mlens_shoot_block.argtypes = [vp, ll, ll, ll, ll, vp, vp, vp, vp]
+    L.mlens_shoot_host.argtypes = [vp, vp, vp, ctypes.POINTER(Stats)]
+    L.mlens_magnification.argtypes = [vp, vp, vp, vp]
+    L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
+    L.mlens_get_stats.argtypes = [vp, vp, ctypes.POINTER(Stats)]
+    L.mlens_reset_stats.argtypes = [vp, vp]
+    L.mlens_set_option.argtypes = [vp, ctypes.c_char_p, ll]
+    L.mlens_last_error.argtypes = []
+    L.mlens_last_error.restype = ctypes.c_char_p
+    L.mlens_destroy.argtypes = [vp]
+    L.mlens_destroy.restype = None
+    for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification",
+                 "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
+        getattr(L, name).restype = ci
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise MlensError(rc, lib().mlens_last_error().decode())
+
+
+def _stream_ptr(stream=None):
+    import torch
+
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+class Mlens:
+    """A map context: mlens_create ... mlens_destroy.  Device tensors are torch tensors on the current CUDA device."""
+
+    def __init__(self, kappa, gamma, s, map_side, npix, ray_spacing, lens_xy, lens_m=None):
+        L = lib()
+        xy = np.ascontiguousarray(np.asarray(lens_xy, dtype=np.float32).reshape(-1))
+        m = None if lens_m is None else np.ascontiguousarray(np.asarray(lens_m, dtype=np.float32).reshape(-1))
+        n = xy.size // 2
+        if m is not None and m.size != n:
+            raise ValueError("lens_m and lens_xy disagree on the number of lenses")
+        self._h = ctypes.c_void_p()
+        self.npix = int(npix)
+        _check(L.mlens_create(ctypes.byref(self._h), kappa, gamma, s, map_side, int(npix), ray_spacing,
+                              xy.ctypes.data_as(ctypes.c_void_p) if n else None,
+                              m.ctypes.data_as(ctypes.c_void_p) if m is not None and n else None, n))
+        g = Geometry()
+        _check(L.mlens_get_geometry(self._h, ctypes.byref(g)))
+        self.geometry = g
+        self.n_lens = n
+
+    @classmethod
+    def from_config(cls, cfg, lens_xy, lens_m):
+        return cls(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, lens_xy, lens_m)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().mlens_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # interpreter shutdown: module globals may already be gone
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def set_option(self, key: str, value: int):
+        _check(lib().mlens_set_option(self._h, key.encode(), int(value)))
+
+    # -- step a1-a5: the whole map -----------------------------------------------------------------------------
+    def shoot(self, count=None, mag=None, want_mag=True, stream=None, sync=True):
+        """mlens_shoot.  Returns (count int32 [npix,npix], mag float32 [npix,npix] or None, stats dict or None)."""
+        import torch
+
+        if count is None:
+            count = torch.empty((self.npix, self.npix), dtype=torch.int32, device="cuda")
+        if mag is None and want_mag:
+            mag = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
+        assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
+        assert mag is None or (mag.is_cuda and mag.dtype == torch.float32 and mag.is_contiguous() and mag.numel() == self.npix**2)
+        st = Stats() if sync else None
+        _check(lib().mlens_shoot(self._h, ctypes.c_void_p(count.data_ptr()),
+                                 ctypes.c_void_p(mag.data_ptr()) if mag is not None else None, _stream_ptr(stream),
+                                 ctypes.byref(st) if sync else None))
+        return count, mag, (st.as_dict() if sync else None)
+
+    # -- verification / partial shooting ---------------------------------------------------------------------------
+    def shoot_block(self, i0, j0, ni, nj, count=None, want_rays=False, stream=None):
+        """mlens_shoot_block.  Returns dict(count, [y float64 (nj,ni,2), pix int32 (nj,ni)]); accumulates into count."""
+        import torch
+
+        y = pix = None
+        if want_rays:
+            y = torch.empty((nj, ni, 2), dtype=torch.float64, device="cuda")
+            pix = torch.empty((nj, ni), dtype=torch.int32, device="cuda")
+        if count is not None:
+            assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
+        _check(lib().mlens_shoot_block(self._h, int(i0), int(j0), int(ni), int(nj),
+                                       ctypes.c_void_p(count.data_ptr()) if count is not None else None,
+                                       ctypes.c_void_p(y.data_ptr()) if y is not None else None,
+                                       ctypes.c_void_p(pix.data_ptr()) if pix is not None else None, _stream_ptr(stream)))
+        return {"count": count, "y": y, "pix": pix}
+
+    def shoot_host(self, want_mag=True):
+        """mlens_shoot_host: HOST numpy buffers in and out (the end-to-end call)."""
+        count = np.empty((self.npix, self.npix), dtype=np.int32)
+        mag = np.empty((self.npix, self.npix), dtype=np.float32) if want_mag else None
+        st = Stats()
+        _check(lib().mlens_shoot_host(self._h, count.ctypes.data_as(ctypes.c_void_p),
+                                      mag.ctypes.data_as(ctypes.c_void_p) if mag is not None else None, ctypes.byref(st)))
+        return count, mag, st.as_dict()
+
+    def magnification(self, count, mag=None, stream=None):
+        import torch
+
+        if mag is None:
+            mag = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
+        _check(lib().mlens_magnification(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(mag.data_ptr()),
+                                         _stream_ptr(stream)))
+        return mag
+
+    def stats(self, stream=None):
+        st = Stats()
+        _check(lib().mlens_get_stats(self._h, _stream_ptr(stream), ctypes.byref(st)))
+        return st.as_dict()
+
+    def reset_stats(self, stream=None):
+        _check(lib().mlens_reset_stats(self._h, _stream_ptr(stream)))

@@ -1,0 +1,252 @@
+"""GPU parity (P10): the CUDA path, through the C ABI, against the FP64 oracle on the same seeded inputs.
+
+Tolerances are BASELINE.json north_star's:
+  (i)   per ray and component |alpha_gpu - alpha_fp64| <= 2e-5 * sum_i m_i/|x - x_i|
+        (checked on y: the macro term is formed identically on both sides, so delta-y = -delta-alpha);
+  (ii)  pixel id bit-exact for every ray whose FP64 source position is > 1e-3 pixel from a pixel edge;
+  (iii) map L1 difference <= 1e-4 of the rays landing in the map.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_1406_0559_b200 import fields
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_ALPHA = 2e-5
+EDGE_BAND = 1e-3
+TOL_L1 = 1e-4
+
+
+@pytest.fixture(scope="module")
+def ml():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1406_0559_b200 import mlens
+
+    mlens.lib()
+    return mlens
+
+
+def _args(cfg):
+    return (cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
+
+
+def check_block(ml, oracle, h, cfg, xy, m, block, acc_gpu=None, acc_ref=None):
+    """Per-ray and per-block comparison; returns dict of counters for aggregation."""
+    i0, j0, ni, nj = block
+    cnt = torch.zeros((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
+    out = h.shoot_block(i0, j0, ni, nj, count=cnt, want_rays=True)
+    torch.cuda.synchronize()
+    y_gpu = out["y"].cpu().numpy()
+    pix_gpu = out["pix"].cpu().numpy()
+    cnt_gpu = cnt.cpu().numpy()
+    ref = oracle.shoot_block(*_args(cfg), xy, m, block=block, want_rays=True)
+    y_ref, pix_ref, scale = ref["y"], ref["pix"], ref["scale"]
+    finite = np.isfinite(y_ref).all(axis=2)
+    # (i) deflection tolerance
+    dy = np.abs(y_gpu - y_ref)
+    bound = TOL_ALPHA * scale[..., None] + 1e-12
+    bad_alpha = int((dy[finite] > np.broadcast_to(bound, dy.shape)[finite]).sum())
+    assert bad_alpha == 0, f"{bad_alpha} deflection components exceed 2e-5*sum(m/r) in block {block}"
+    assert np.array_equal(pix_gpu == -2, ~finite)
+    # (ii) pixel assignment away from edges
+    u = (y_ref + cfg.map_side / 2.0) / cfg.pixel
+    dist = np.abs(u - np.round(u)).min(axis=2)
+    far = finite & (dist > EDGE_BAND)
+    mism_far = int((pix_gpu[far] != pix_ref[far]).sum())
+    assert mism_far == 0, f"{mism_far} rays > 1e-3 px from an edge got a different pixel in block {block}"
+    mism_all = int((pix_gpu != pix_ref).sum())
+    # block map == histogram of the block's own pixel ids (binning is exact integer work)
+    hist = np.bincount(pix_gpu[pix_gpu >= 0].ravel(), minlength=cfg.npix**2).reshape(cfg.npix, cfg.npix)
+    assert np.array_equal(hist, cnt_gpu)
+    if acc_gpu is not None:
+        acc_gpu += cnt_gpu
+        acc_ref += ref["count"]
+    # error in pixels for the record
+    err_px = (dy[finite] / cfg.pixel)
+    return {"rays": ni * nj, "in_map": ref["stats"]["rays_in_map"], "mismatch": mism_all,
+            "l1": int(np.abs(cnt_gpu.astype(np.int64) - ref["count"]).sum()),
+            "mean_err_px": float(err_px.mean()) if err_px.size else 0.0, "max_err_px": float(err_px.max()) if err_px.size else 0.0}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# closed forms and edge cases through the CUDA path
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [1, 0])
+def test_no_lens_uniform_map_is_exact(ml, oracle, kernel):
+    # P1(b) through the GPU: kappa=0.3, gamma=0.2, all smooth: counts {220, 240}, mean 222.5 — exact integers
+    L, npix, sub = 4.0, 64, 10
+    with ml.Mlens(0.3, 0.2, 1.0, L, npix, L / npix / sub, np.zeros((0, 2), np.float32)) as h:
+        h.set_option("kernel", kernel)
+        count, mag, st = h.shoot()
+    c = count.cpu().numpy()
+    assert set(np.unique(c).tolist()) == {220, 240} and c.mean() == 222.5
+    ref = oracle.shoot_block(0.3, 0.2, 1.0, L, npix, L / npix / sub, np.zeros((0, 2), np.float32), None)
+    assert np.array_equal(c, ref["count"])
+    assert st["rays_total"] == ref["stats"]["rays_total"] and st["rays_in_map"] == ref["stats"]["rays_in_map"]
+    assert st["rays_lost"] == 0 and st["max_count"] == 240
+    assert np.array_equal(mag.cpu().numpy(), oracle.magnification(c, 100.0))
+
+
+def test_tiny_config_full_map(ml, oracle):
+    # configs[0]: the whole map against the oracle (2.1e7 rays, 13 lenses; ragged n2 = 3414 = 53*64 + 22)
+    cfg = fields.CONFIGS[1]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        assert (h.geometry.n1, h.geometry.n2) == (6144, 3414)
+        count, mag, st = h.shoot()
+        host_count, host_mag, host_st = h.shoot_host()
+    ref = oracle.shoot_block(*_args(cfg), xy, m)
+    c = count.cpu().numpy()
+    l1 = int(np.abs(c.astype(np.int64) - ref["count"]).sum())
+    assert st["rays_total"] == ref["stats"]["rays_total"] == 6144 * 3414
+    assert st["rays_in_map"] + st["rays_outside"] + st["rays_lost"] == st["rays_total"]
+    assert int(c.sum(dtype=np.int64)) == st["rays_in_map"]
+    assert abs(st["rays_in_map"] - ref["stats"]["rays_in_map"]) <= l1
+    assert l1 <= TOL_L1 * ref["stats"]["rays_in_map"], (l1, ref["stats"]["rays_in_map"])
+    assert st["max_count"] == int(c.max())
+    assert np.array_equal(mag.cpu().numpy(), oracle.magnification(c, ref["geometry"].n_avg))
+    # host-buffer entry point gives the same map (integer REDs: order-independent => deterministic)
+    assert np.array_equal(host_count, c) and np.array_equal(host_mag, mag.cpu().numpy())
+    assert host_st["rays_in_map"] == st["rays_in_map"]
+
+
+def test_ragged_and_degenerate_blocks(ml, oracle):
+    cfg = dataclasses.replace(fields.CONFIGS[1], npix=128, sub=6)
+    xy, m = fields.random_field(40, cfg.disc_radius, 5, "salpeter")
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        n1, n2 = h.geometry.n1, h.geometry.n2
+        blocks = [(0, 0, 1, 1), (n1 - 1, n2 - 1, 1, 1), (3, 5, 64, 64), (7, 11, 65, 63), (0, 0, 200, 3), (n1 - 130, 0, 130, 257),
+                  (0, n2 - 77, n1, 77), (n1 // 2 - 100, n2 // 2 - 100, 201, 199)]
+        for b in blocks:
+            r = check_block(ml, oracle, h, cfg, xy, m, b)
+            assert r["l1"] <= max(2, 2 * r["mismatch"])
+        # empty block: no work, no error; out-of-range block: EINVAL
+        h.shoot_block(5, 5, 0, 0)
+        with pytest.raises(ml.MlensError):
+            h.shoot_block(0, 0, n1 + 1, 1)
+        with pytest.raises(ml.MlensError):
+            h.shoot_block(-1, 0, 1, 1)
+
+
+def test_ray_exactly_on_a_lens_is_lost(ml, oracle):
+    L, npix, sub = 4.0, 16, 2
+    d = L / npix / sub
+    g = oracle.geometry(0.0, 0.0, 0.0, L, npix, d)
+    x_on_ray = np.array([[(5 + 0.5 - g.n1 / 2) * d, (9 + 0.5 - g.n2 / 2) * d]], np.float32)
+    with ml.Mlens(0.0, 0.0, 0.0, L, npix, d, x_on_ray) as h:
+        count, _, st = h.shoot()
+        out = h.shoot_block(0, 0, g.n1, g.n2, want_rays=True)
+    ref = oracle.shoot_block(0.0, 0.0, 0.0, L, npix, d, x_on_ray, None, want_rays=True)
+    assert st["rays_lost"] == ref["stats"]["rays_lost"] == 1
+    assert out["pix"].cpu().numpy()[9, 5] == -2
+    assert np.array_equal(count.cpu().numpy(), ref["count"])
+
+
+def test_multi_chunk_lens_list(ml, oracle):
+    # N* > 3072 streams the list through shared memory in 2048-lens chunks (double-buffered bulk copies)
+    cfg = fields.MapConfig("chunks", 128, 6.0, 0.55, 0.1, 0.0, 4, "salpeter", 31)
+    xy, m = fields.random_field(5000, 60.0, 31, "salpeter")
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        n1, n2 = h.geometry.n1, h.geometry.n2
+        tot = {"in_map": 0, "l1": 0}
+        for b in [(0, 0, 256, 192), (n1 // 2 - 128, n2 // 2 - 96, 256, 192), (n1 - 200, n2 - 130, 200, 130)]:
+            r = check_block(ml, oracle, h, cfg, xy, m, b)
+            tot["in_map"] += r["in_map"]; tot["l1"] += r["l1"]
+    assert tot["l1"] <= max(4, TOL_L1 * tot["in_map"])
+
+
+def test_binning_variants_and_fp64_kernel_agree(ml, oracle):
+    cfg = dataclasses.replace(fields.CONFIGS[1], npix=192, sub=5)
+    xy, m = fields.lens_field(cfg)
+    maps = {}
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        for mode in (0, 1, 2, 3):
+            h.set_option("binning", mode)
+            count, _, st = h.shoot(want_mag=False)
+            maps[mode] = (count.cpu().numpy().copy(), st)
+        h.set_option("kernel", 0)
+        c64, _, st64 = h.shoot(want_mag=False)
+        c64 = c64.cpu().numpy()
+    for mode in (1, 2, 3):  # same per-ray pixels, different routes to the map: bit-identical
+        assert np.array_equal(maps[mode][0], maps[0][0]), mode
+        assert maps[mode][1]["rays_in_map"] == maps[0][1]["rays_in_map"]
+    ref = oracle.shoot_block(*_args(cfg), xy, m)
+    in_map = ref["stats"]["rays_in_map"]
+    assert np.abs(c64.astype(np.int64) - ref["count"]).sum() <= max(2, 1e-6 * in_map)  # FP64 kernel ~ oracle
+    assert np.abs(maps[1][0].astype(np.int64) - ref["count"]).sum() <= TOL_L1 * in_map
+
+
+def test_mirror_symmetry_on_gpu(ml):
+    # P6 through the CUDA path
+    cfg = dataclasses.replace(fields.CONFIGS[1], npix=128, sub=6)
+    xy, m = fields.random_field(30, cfg.disc_radius, 9, "salpeter")
+    xm = xy.copy(); xm[:, 0] = -xm[:, 0]
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        a, _, st = h.shoot(want_mag=False)
+    with ml.Mlens.from_config(cfg, xm, m) as h:
+        b, _, _ = h.shoot(want_mag=False)
+    a, b = a.cpu().numpy().astype(np.int64), b.cpu().numpy().astype(np.int64)
+    assert np.abs(a - b[:, ::-1]).sum() <= 2e-4 * st["rays_in_map"]
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the five configurations: seeded sub-blocks (random, lens-centred, border) + full-map invariants
+# ---------------------------------------------------------------------------------------------------------------
+N_BLOCKS = {1: (8, 6, 4), 2: (6, 4, 2), 3: (12, 8, 4), 4: (12, 8, 4), 5: (12, 8, 4)}
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2, 3, 4, 5])
+def test_config_sub_blocks(ml, oracle, cfg_id):
+    cfg = fields.CONFIGS[cfg_id]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        g = h.geometry
+        nr, nl, nb = N_BLOCKS[cfg_id]
+        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed, nr, nl, nb, size=256)
+        acc_gpu = np.zeros((cfg.npix, cfg.npix), np.int64)
+        acc_ref = np.zeros((cfg.npix, cfg.npix), np.int64)
+        tot = {"rays": 0, "in_map": 0, "mismatch": 0, "mean_err_px": 0.0, "max_err_px": 0.0}
+        for b in blocks:
+            r = check_block(ml, oracle, h, cfg, xy, m, b, acc_gpu, acc_ref)
+            tot["rays"] += r["rays"]; tot["in_map"] += r["in_map"]; tot["mismatch"] += r["mismatch"]
+            tot["mean_err_px"] += r["mean_err_px"] * r["rays"]; tot["max_err_px"] = max(tot["max_err_px"], r["max_err_px"])
+    l1 = int(np.abs(acc_gpu - acc_ref).sum())
+    print(f"cfg{cfg_id}: {len(blocks)} blocks, {tot['rays']} rays, in_map {tot['in_map']}, pixel mismatches {tot['mismatch']}, "
+          f"L1 {l1} ({l1 / max(1, tot['in_map']):.2e}), mean|err| {tot['mean_err_px'] / tot['rays']:.2e} px, max {tot['max_err_px']:.2e} px")
+    assert l1 <= max(4, TOL_L1 * tot["in_map"]), (l1, tot)
+
+
+@pytest.mark.parametrize("cfg_id", [3, 4, 5])
+def test_full_map_invariants(ml, oracle, cfg_id):
+    # the launch configuration bench.py times: whole lattice, default options
+    cfg = fields.CONFIGS[cfg_id]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        g = h.geometry
+        count, mag, st = h.shoot()
+        assert st["rays_total"] == g.n1 * g.n2
+        assert st["rays_in_map"] + st["rays_outside"] + st["rays_lost"] == st["rays_total"]
+        assert int(count.sum(dtype=torch.int64).item()) == st["rays_in_map"]
+        assert st["max_count"] == int(count.max().item()) and st["max_count"] < 2**31 - 1
+        # magnification: bit-exact Eq. 4 on sampled pixels
+        idx = (fields.uniform01(cfg.seed + 5, 0, 4096) * cfg.npix**2).astype(np.int64)
+        c_s = count.view(-1)[torch.from_numpy(idx).cuda()].cpu().numpy()
+        m_s = mag.view(-1)[torch.from_numpy(idx).cuda()].cpu().numpy()
+        assert np.array_equal(m_s, oracle.magnification(c_s, g.n_avg))
+        # sampled rays, one by one, against the oracle: per-ray pixel ids via 1x1 blocks are too slow; use 64 8x8 blocks
+        u = fields.uniform01(cfg.seed + 6, 0, 128)
+        mism = 0
+        for k in range(64):
+            i0, j0 = int(u[2 * k] * (g.n1 - 8)), int(u[2 * k + 1] * (g.n2 - 8))
+            r = check_block(ml, oracle, h, cfg, xy, m, (i0, j0, 8, 8))
+            mism += r["mismatch"]
+        assert mism <= 2
+    mean_mu = st["rays_in_map"] / (cfg.npix**2 * cfg.sub**2)
+    print(f"cfg{cfg_id}: full map {st['elapsed_ms']:.1f} ms, <mu>/mu_th = {mean_mu / cfg.mu_th:.4f}, max count {st['max_count']}")
+    if cfg_id in (3, 5):
+        assert abs(mean_mu / cfg.mu_th - 1) < 0.15
