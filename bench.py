@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the direct inverse ray-shooting hot path (BASELINE.json metric) on B200.
+
+A "step" is one pass of the whole hot path (lattice, deflection sum over all N* lenses,
+source position, binning, count -> magnification) over one synthetic map.  The default workload is BASELINE.json's
+config 4 (`configs[3]`, the near-critical 1024^2 field the north_star quotes its FP32 target on); `--config` selects
+another.  One JSON line is printed by rank 0.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+* `value`      ray-lens interactions/s, all ranks, device-timed (CUDA events on the launching stream), max over ranks.
+* `e2e`        the same metric through `mlens_create` + `mlens_shoot_host` + `mlens_destroy` with HOST buffers (lens
+               arrays in, count + magnification maps out), copies inside the timed region.
+* `roofline`   the shooting kernel alone: 11 flops x interactions / kernel time (events inside libmlens around the
+               kernel launch) against the FP32 peak SMs x 128 x 2 x f_max; bound = "alu".
+* `cpu_baseline` the FP64 oracle (oracle/) on the box's host cores on a bounded block of the same lattice.
+* N > 1        weak scaling: every rank shoots an independent map of the same config (seed + rank), the way the paper
+               scales (one map per GPU); no data-path collective.
+* `--impl reference`  times the oracle, as it stands, on the host cores (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1406_0559_b200 import fields  # noqa: E402
+
+METRIC = "ray_lens_interactions_per_s"
+UNIT = "interactions/s"
+FLOPS_PER_INTERACTION = 11  # 2 sub, mul+fma (r^2), rcp, mass mul, 2 fma (10 when all m_i = 1)
+FP32_LANES_PER_SM = 128
+
+
+def flops_per_interaction(cfg) -> int:
+    return FLOPS_PER_INTERACTION if cfg.masses != "unit" else FLOPS_PER_INTERACTION - 1
+
+
+def workload_name(cfg_id: int, cfg, n_lens: int, n1: int, n2: int) -> str:
+    return (f"BASELINE.json config {cfg_id} ({cfg.name}): {cfg.npix}^2 px, side {cfg.map_side:g} R_E, kappa={cfg.kappa:g}, "
+            f"gamma={cfg.gamma:g}, s={cfg.s:g}, spacing=pixel/{cfg.sub}, masses={cfg.masses}, N*={n_lens}, "
+            f"lattice {n1}x{n2}")
+
+
+# -----------------------------------------------------------------------------------------------------------------
+# clocks
+# -----------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(smax), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# -----------------------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): the ONLY places bench.py touches oracle/
+# -----------------------------------------------------------------------------------------------------------------
+def oracle_block_for(cfg, n1, n2, n_lens, target_s, rate_guess):
+    """A centred ni x nj block of the config's lattice holding about target_s seconds of oracle work."""
+    rays = max(4096.0, target_s * rate_guess / max(1, n_lens))
+    side = int(max(64, min(min(n1, n2), round(rays**0.5))))
+    return ((n1 - side) // 2, (n2 - side) // 2, side, side)
+
+
+def oracle_time_block(oracle, cfg, xy, m, block):
+    t0 = time.perf_counter()
+    r = oracle.shoot_block(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, xy, m, block=block)
+    dt = time.perf_counter() - t0
+    return dt, r["stats"]["rays_total"]
+
+
+def oracle_calibrate(oracle, cfg, xy, m, n1, n2):
+    """Rate (interactions/s) from a short run, used only to SIZE the timed sample."""
+    n_lens = max(1, len(m))
+    blk = oracle_block_for(cfg, n1, n2, n_lens, 1.0, 2.0e9)
+    dt, rays = oracle_time_block(oracle, cfg, xy, m, blk)
+    return rays * n_lens / max(dt, 1e-6)
+
+
+def run_cpu_baseline(cfg, xy, m, target_s=15.0):
+    import oracle
+
+    oracle.lib()
+    g = oracle.geometry(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
+    n_lens = max(1, len(m))
+    rate0 = oracle_calibrate(oracle, cfg, xy, m, g.n1, g.n2)
+    blk = oracle_block_for(cfg, g.n1, g.n2, n_lens, target_s, rate0)
+    dt, rays = oracle_time_block(oracle, cfg, xy, m, blk)
+    return {"value": rays * n_lens / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "rays_per_s": rays / dt, "seconds": dt,
+            "sample": f"centred {blk[2]}x{blk[3]}-ray block of the same lattice ({rays} rays x {n_lens} lenses = "
+                      f"{rays * n_lens:.3e} interactions), FP64 C++ -O3 -march=native, OpenMP, oracle/oracle.cpp as it stands"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, K timed steps of a bounded sample each (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+
+    oracle.lib()
+    cfg = fields.CONFIGS[args.config]
+    xy, m = fields.lens_field(cfg)
+    g = oracle.geometry(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
+    n_lens = max(1, len(m))
+    rate0 = oracle_calibrate(oracle, cfg, xy, m, g.n1, g.n2)
+    per_step = min(8.0, 120.0 / max(1, args.steps + args.warmup))
+    blk = oracle_block_for(cfg, g.n1, g.n2, n_lens, per_step, rate0)
+    for _ in range(args.warmup):
+        oracle_time_block(oracle, cfg, xy, m, blk)
+    t0 = time.perf_counter()
+    rays = 0
+    for _ in range(args.steps):
+        _, r = oracle_time_block(oracle, cfg, xy, m, blk)
+        rays += r
+    dt = time.perf_counter() - t0
+    value = rays * n_lens / dt
+    sample = (f"each step: centred {blk[2]}x{blk[3]}-ray block of the config's lattice ({blk[2] * blk[3] * n_lens:.3e} "
+              f"interactions), FP64 oracle on host cores")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, cfg, len(m), g.n1, g.n2), "sample": sample},
+            "rays_per_s": rays / dt,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# -----------------------------------------------------------------------------------------------------------------
+# our arm
+# -----------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1406_0559_b200 import mlens
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    mlens.lib()  # fail loudly if libmlens.so is missing
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    import dataclasses
+
+    cfg0 = fields.CONFIGS[args.config]
+    cfg = dataclasses.replace(cfg0, seed=cfg0.seed + rank)  # weak scaling: an independent map per rank
+    xy, m = fields.lens_field(cfg)
+    n_lens = len(m)
+    h = mlens.Mlens.from_config(cfg, xy, m)
+    g = h.geometry
+    rays = g.n1 * g.n2
+    inter = rays * max(1, n_lens)
+    count = torch.empty((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
+    mag = torch.empty((cfg.npix, cfg.npix), dtype=torch.float32, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    def step(sync_stats=False):
+        flush.fill_(1)  # evict the count map and lens list from L2 between steps
+        return h.shoot(count=count, mag=mag, sync=sync_stats)[2]
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    kernel_ms = []
+    for _ in range(args.steps):
+        st = step(sync_stats=True)  # stats pointer => libmlens brackets the shooting kernel with its own events
+        kernel_ms.append(st["kernel_ms"])
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms_total, sum(kernel_ms) / max(1, len(kernel_ms))], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, kern_ms = float(t[0]), float(t[1])
+    assert st["rays_total"] == rays and st["rays_in_map"] + st["rays_outside"] + st["rays_lost"] == rays
+    in_map = st["rays_in_map"]
+
+    # end to end through the C ABI with host buffers: create (H2D lens list) + shoot + D2H maps + destroy
+    e2e_steps = max(1, min(args.steps, 2))
+    h.close()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        with mlens.Mlens.from_config(cfg, xy, m) as h2:
+            c_host, m_host, st2 = h2.shoot_host()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t[0])
+    assert int(c_host.sum(dtype=np.int64)) == st2["rays_in_map"] == in_map
+
+    if rank == 0:
+        prop = torch.cuda.get_device_properties(local_rank)
+        sms = prop.multi_processor_count
+        f_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        peak = sms * FP32_LANES_PER_SM * 2 * f_max_mhz * 1e6 / 1e12  # TFLOP/s at the maximum SM clock
+        fpi = flops_per_interaction(cfg)
+        achieved = fpi * inter / (kern_ms * 1e-3) / 1e12
+        value = world * inter * args.steps / (ms_total * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_total / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, cfg0, n_lens, g.n1, g.n2), "rays_per_map": rays,
+                       "interactions_per_map": inter, "rays_in_map": in_map,
+                       "l2": "256 MiB device write between steps (inputs are smaller than L2)",
+                       "parallelism": f"{world} independent map(s), one per GPU (seed + rank)"},
+            "rays_per_s": world * rays * args.steps / (ms_total * 1e-3),
+            "clocks": clocks,
+            "e2e": {"value": world * inter * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
+                    "h2d_bytes_per_step": int(xy.nbytes + m.nbytes), "d2h_bytes_per_step": int(c_host.nbytes + m_host.nbytes)},
+            "gpu_launches": 2 * args.steps,  # shoot_fp32_kernel + magnification_kernel per step (memsets are driver ops)
+            "roofline": {"bound": "alu", "kernel": "shoot_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": None, "flops_per_interaction": fpi,
+                         "kernel_ms": kern_ms,
+                         "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 x {f_max_mhz:.0f} MHz (clocks.max.sm); "
+                                        "no FP32 figure in MEASURED_PEAKS.json",
+                         "mufu_ceiling_frac": 16.0 * fpi / (FP32_LANES_PER_SM * 2)},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = run_cpu_baseline(cfg, xy, m)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_block(args):
+    """--block S: K launches of mlens_shoot_block on a centred S x S-ray block (the short launch ncu profiles)."""
+    import torch
+
+    from paper_1406_0559_b200 import mlens
+
+    torch.cuda.set_device(0)
+    cfg = fields.CONFIGS[args.config]
+    xy, m = fields.lens_field(cfg)
+    with mlens.Mlens.from_config(cfg, xy, m) as h:
+        for k, v in (args.option or []):
+            h.set_option(k, int(v))
+        g = h.geometry
+        si, sj = min(args.block, g.n1), min(args.block, g.n2)
+        blk = ((g.n1 - si) // 2, (g.n2 - sj) // 2, si, sj)
+        count = torch.zeros((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
+        for _ in range(args.warmup):
+            h.shoot_block(*blk, count=count)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        ev[0].record()
+        for k in range(args.steps):
+            h.shoot_block(*blk, count=count)
+            ev[k + 1].record()
+        torch.cuda.synchronize()
+        ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+        st = h.stats()
+    inter = si * sj * max(1, len(m))
+    med = statistics.median(ms)
+    fpi = flops_per_interaction(cfg)
+    print(json.dumps({"mode": "block", "config": args.config, "block": blk, "options": args.option, "ms": ms, "ms_median": med,
+                      "interactions_per_s": inter / (med * 1e-3), "rays_per_s": si * sj / (med * 1e-3),
+                      "tflops": fpi * inter / (med * 1e-3) / 1e12,
+                      "frac_fp32_peak_1965": fpi * inter / (med * 1e-3) / (148 * 128 * 2 * 1.965e9),
+                      "rays_in_map_frac": st["rays_in_map"] / max(1, st["rays_total"])}), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(fields.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
+    ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
+    args = ap.parse_args()
+    if args.block:
+        run_block(args)
+    elif args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -48,6 +48,7 @@ typedef struct {
     int max_count;          /* largest pixel count seen by the last mlens_shoot / mlens_magnification (overflow guard,
                                PAPER.md:692-698: the paper's largest observed count is 998 878) */
     float elapsed_ms;       /* device time of the last mlens_shoot that was given a stats pointer, else 0 */
+    float kernel_ms;        /* of which: the shooting kernel alone (steps a1-a4), CUDA events on `cuda_stream` */
 } mlens_stats;
 
 typedef struct {

@@ -14,8 +14,26 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-fPIC", "-Xptxas", "-v"]
 
 
+MICRO_SRC = os.path.join(_HERE, "csrc", "alu_microbench.cu")
+MICRO_OUT = os.path.join(_HERE, "lib", "alu_microbench")
+
+
+def build_microbench(force: bool = False) -> str:
+    """The pipe-rate microbenchmark executable; not on the product path."""
+    os.makedirs(os.path.dirname(MICRO_OUT), exist_ok=True)
+    if force or not os.path.exists(MICRO_OUT) or os.path.getmtime(MICRO_OUT) < os.path.getmtime(MICRO_SRC):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-o", MICRO_OUT, MICRO_SRC]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    return MICRO_OUT
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(os.path.dirname(OUT), exist_ok=True)
+    build_microbench(force)
     stale = force or not os.path.exists(OUT) or any(os.path.getmtime(OUT) < os.path.getmtime(d) for d in DEPS)
     if stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

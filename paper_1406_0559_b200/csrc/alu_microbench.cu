@@ -1,0 +1,184 @@
+// alu_microbench.cu — register-only pipe-rate microbenchmarks for sm_100a.
+//
+// MEASURED_PEAKS.json holds HBM and bf16 tensor peaks only; the shooting kernel is bound by the plain ALUs
+// (FP32 FMA pipe, MUFU pipe, issue slots).  This program measures, per SM sub-partition (SMSP), how many warp-wide
+// instructions per clock each instruction mix sustains, with the SM clock read from clock64() inside the kernel and
+// the wall time from CUDA events (their ratio is the SM frequency during the run).
+//
+// Build:  nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -o alu_microbench alu_microbench.cu
+// Run:    ./alu_microbench            (prints one JSON object)
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+#define CK(x)                                                                             \
+    do {                                                                                  \
+        cudaError_t e_ = (x);                                                             \
+        if (e_ != cudaSuccess) {                                                          \
+            fprintf(stderr, "%s: %s\n", #x, cudaGetErrorString(e_));                      \
+            exit(1);                                                                      \
+        }                                                                                 \
+    } while (0)
+
+constexpr int kIters = 4096;
+constexpr int kChains = 16;
+
+__device__ __forceinline__ float rcp_mufu(float x) {
+    float r;
+    asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, N_MIX };
+static const char* kMixName[N_MIX] = {"ffma", "ffma2", "mufu_rcp", "ffma4_mufu1", "kernel_mix_6ffma2_2mufu",
+                                      "paired_mix_6ffma2_3fmul_1mufu", "dfma", "fadd2", "lds128_broadcast"};
+// warp-instructions issued per inner iteration per thread, FP32 flops per iteration per thread
+static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains};
+
+template <int MIX>
+__global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycles, float seed) {
+    __shared__ float4 sm[256];
+    sm[threadIdx.x] = make_float4(seed, seed * 0.5f, seed * 0.25f, 1.0f);
+    __syncthreads();
+    float a[kChains];
+    float2 p[kChains / 2], s2[kChains / 2];
+    double dd[kChains];
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) {
+        a[k] = seed + 0.001f * (float)(k + threadIdx.x);
+        dd[k] = (double)a[k];
+    }
+#pragma unroll
+    for (int k = 0; k < kChains / 2; ++k) { p[k] = make_float2(a[2 * k], a[2 * k + 1]); s2[k] = make_float2(0.f, 0.f); }
+    const float b = 0.999f + seed * 1e-6f, c = seed * 1e-3f;
+    const float2 b2 = make_float2(b, b), c2 = make_float2(c, c);
+    const long long t0 = clock64();
+    for (int it = 0; it < kIters; ++it) {
+        if (MIX == FFMA) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) a[k] = fmaf(a[k], b, c);
+        } else if (MIX == FFMA2) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) p[k] = __ffma2_rn(p[k], b2, c2);
+        } else if (MIX == FADD2_ONLY) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) p[k] = __fadd2_rn(p[k], c2);
+        } else if (MIX == MUFU) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k)  // the LOP3 (ALU pipe) keeps nvcc from folding rcp(rcp(x)) to x
+                a[k] = __int_as_float(__float_as_int(rcp_mufu(a[k])) ^ 1);
+        } else if (MIX == FFMA_MUFU_41) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                a[k] = rcp_mufu(a[k]);
+                a[4 + k] = fmaf(a[4 + k], b, c);
+                a[8 + k] = fmaf(a[8 + k], b, c);
+                a[12 + k] = fmaf(a[12 + k], b, a[k]);
+                a[k] = fmaf(a[k], b, c);
+            }
+        } else if (MIX == KERNEL_MIX) {
+            // the difference-form interaction for 8 ray pairs: 1 FADD2 + 5 FFMA2 + 2 MUFU per pair
+#pragma unroll
+            for (int k = 0; k < kChains / 2; ++k) {
+                const float2 dx = __fadd2_rn(p[k], c2);
+                const float2 r2 = __ffma2_rn(dx, dx, b2);
+                const float2 rc = make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y));
+                const float2 pr = __ffma2_rn(b2, dx, c2);
+                const float2 pi = __ffma2_rn(c2, dx, b2);
+                p[k] = __ffma2_rn(pr, rc, p[k]);
+                s2[k] = __ffma2_rn(pi, rc, s2[k]);
+            }
+        } else if (MIX == PAIRED_MIX) {
+            // one reciprocal per ray pair: rc = 1/(r2.x*r2.y); 1/r2.x = rc*r2.y, 1/r2.y = rc*r2.x
+#pragma unroll
+            for (int k = 0; k < kChains / 2; ++k) {
+                const float2 dx = __fadd2_rn(p[k], c2);
+                const float2 r2 = __ffma2_rn(dx, dx, b2);
+                const float q = rcp_mufu(r2.x * r2.y);
+                const float2 rc = make_float2(q * r2.y, q * r2.x);
+                const float2 pr = __ffma2_rn(b2, dx, c2);
+                const float2 pi = __ffma2_rn(c2, dx, b2);
+                p[k] = __ffma2_rn(pr, rc, p[k]);
+                s2[k] = __ffma2_rn(pi, rc, s2[k]);
+            }
+        } else if (MIX == DFMA) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) dd[k] = fma(dd[k], (double)b, (double)c);
+        } else if (MIX == LDS128) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) {
+                const float4 q = sm[(it * kChains + k) & 255];  // same address in every lane: broadcast
+                a[k] += q.x + q.w;
+            }
+        }
+    }
+    const long long t1 = clock64();
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) s += a[k] + (float)dd[k];
+#pragma unroll
+    for (int k = 0; k < kChains / 2; ++k) s += p[k].x + p[k].y + s2[k].x + s2[k].y;
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+template <int MIX>
+void run(int sms, int ctas_per_sm, float* out, long long* cyc_dev, bool last) {
+    const int grid = sms * ctas_per_sm;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);  // warm-up
+    CK(cudaDeviceSynchronize());
+    float best = 1e30f;
+    long long cyc_best = 0;
+    for (int rep = 0; rep < 5; ++rep) {
+        CK(cudaEventRecord(e0));
+        bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        float ms;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        long long c0;
+        CK(cudaMemcpy(&c0, cyc_dev, sizeof(c0), cudaMemcpyDeviceToHost));
+        if (ms < best) { best = ms; cyc_best = c0; }
+    }
+    // warp-instructions per clock per SMSP from the in-kernel cycle count of CTA 0
+    const double warps_per_smsp = ctas_per_sm * 8 / 4.0;
+    const double instr = (double)kIters * kInstr[MIX] * warps_per_smsp;
+    const double ipc = instr / (double)cyc_best;
+    const double mhz = (double)cyc_best / (best * 1e-3) * 1e-6;
+    printf("  \"%s\": {\"ctas_per_sm\": %d, \"warp_instr_per_clk_per_smsp\": %.4f, \"cycles\": %lld, \"ms\": %.4f, \"sm_mhz_upper\": %.0f}%s\n",
+           kMixName[MIX], ctas_per_sm, ipc, cyc_best, best, mhz, last ? "" : ",");
+    CK(cudaEventDestroy(e0));
+    CK(cudaEventDestroy(e1));
+}
+
+int main(int argc, char** argv) {
+    int ctas = argc > 1 ? atoi(argv[1]) : 4;
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, 0));
+    const int sms = prop.multiProcessorCount;
+    float* out;
+    long long* cyc;
+    CK(cudaMalloc(&out, sizeof(float) * sms * 8 * 256));
+    CK(cudaMalloc(&cyc, sizeof(long long) * sms * 8));
+    printf("{\n  \"device\": \"%s\", \"sms\": %d, \"clock_rate_khz\": %d,\n", prop.name, sms, prop.clockRate);
+    run<FFMA>(sms, ctas, out, cyc, false);
+    run<FFMA2>(sms, ctas, out, cyc, false);
+    run<FADD2_ONLY>(sms, ctas, out, cyc, false);
+    run<MUFU>(sms, ctas, out, cyc, false);
+    run<FFMA_MUFU_41>(sms, ctas, out, cyc, false);
+    run<KERNEL_MIX>(sms, ctas, out, cyc, false);
+    run<PAIRED_MIX>(sms, ctas, out, cyc, false);
+    run<DFMA>(sms, ctas, out, cyc, false);
+    run<LDS128>(sms, ctas, out, cyc, true);
+    printf("}\n");
+    return 0;
+}

@@ -56,8 +56,8 @@ struct mlens {
     int* count_own;
     float* mag_own;
     cudaStream_t own_stream;
-    cudaEvent_t ev0, ev1;
-    float last_ms;
+    cudaEvent_t ev0, ev1, evk0, evk1;
+    float last_ms, last_kernel_ms;
     // options
     int opt_kernel, opt_binning, opt_ctas_per_sm;
 };
@@ -144,6 +144,7 @@ int read_stats(mlens_t* h, cudaStream_t st, mlens_stats* out) {
     memcpy(&mc, h->counters_host + 4, sizeof(int));
     out->max_count = mc;
     out->elapsed_ms = h->last_ms;
+    out->kernel_ms = h->last_kernel_ms;
     return MLENS_OK;
 }
 
@@ -216,6 +217,8 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     if (e == cudaSuccess) e = cudaMallocHost(&h->counters_host, 8 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaEventCreate(&h->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&h->ev1);
+    if (e == cudaSuccess) e = cudaEventCreate(&h->evk0);
+    if (e == cudaSuccess) e = cudaEventCreate(&h->evk1);
     if (e != cudaSuccess) {
         const int code = fail(e == cudaErrorMemoryAllocation ? MLENS_ENOMEM : MLENS_ECUDA, "mlens_create: %s", cudaGetErrorString(e));
         mlens_destroy(h);
@@ -236,6 +239,8 @@ void mlens_destroy(mlens_t* h) {
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
+    if (h->evk0) cudaEventDestroy(h->evk0);
+    if (h->evk1) cudaEventDestroy(h->evk1);
     delete h;
 }
 
@@ -294,12 +299,15 @@ int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, m
     if (stats) MLENS_CUDA(cudaEventRecord(h->ev0, st));
     MLENS_CUDA(cudaMemsetAsync(count_dev, 0, n * sizeof(int), st));
     MLENS_CUDA(cudaMemsetAsync(h->counters_dev, 0, 4 * sizeof(unsigned long long), st));
+    if (stats) MLENS_CUDA(cudaEventRecord(h->evk0, st));
     if (int rc = launch_block(h, 0, 0, h->geo.n1, h->geo.n2, count_dev, nullptr, nullptr, st)) return rc;
+    if (stats) MLENS_CUDA(cudaEventRecord(h->evk1, st));
     if (int rc = launch_magnification(h, count_dev, mag_dev, st)) return rc;
     if (stats) {
         MLENS_CUDA(cudaEventRecord(h->ev1, st));
         MLENS_CUDA(cudaEventSynchronize(h->ev1));
         MLENS_CUDA(cudaEventElapsedTime(&h->last_ms, h->ev0, h->ev1));
+        MLENS_CUDA(cudaEventElapsedTime(&h->last_kernel_ms, h->evk0, h->evk1));
         return read_stats(h, st, stats);
     }
     return MLENS_OK;

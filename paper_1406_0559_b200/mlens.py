@@ -27,7 +27,7 @@ class MlensError(RuntimeError):
 class Stats(ctypes.Structure):
     _fields_ = [("rays_total", ctypes.c_longlong), ("rays_in_map", ctypes.c_longlong),
                 ("rays_outside", ctypes.c_longlong), ("rays_lost", ctypes.c_longlong), ("n_lens", ctypes.c_longlong),
-                ("max_count", ctypes.c_int), ("elapsed_ms", ctypes.c_float)]
+                ("max_count", ctypes.c_int), ("elapsed_ms", ctypes.c_float), ("kernel_ms", ctypes.c_float)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
