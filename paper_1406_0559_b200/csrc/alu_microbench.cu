@@ -22,7 +22,7 @@
         }                                                                                 \
     } while (0)
 
-constexpr int kIters = 4096;
+constexpr int kIters = 16384;
 constexpr int kChains = 16;
 
 __device__ __forceinline__ float rcp_mufu(float x) {
@@ -31,11 +31,12 @@ __device__ __forceinline__ float rcp_mufu(float x) {
     return r;
 }
 
-enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, N_MIX };
+enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, FFMA2_FMUL, FFMA2_MUFU_INDEP, N_MIX };
 static const char* kMixName[N_MIX] = {"ffma", "ffma2", "mufu_rcp", "ffma4_mufu1", "kernel_mix_6ffma2_2mufu",
-                                      "paired_mix_6ffma2_3fmul_1mufu", "dfma", "fadd2", "lds128_broadcast"};
+                                      "paired_mix_6ffma2_3fmul_1mufu", "dfma", "fadd2", "lds128_broadcast",
+                                      "ffma2x12_fmulx6", "ffma2x12_mufux4_independent"};
 // warp-instructions issued per inner iteration per thread, FP32 flops per iteration per thread
-static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains};
+static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains, 18, 16};
 
 template <int MIX>
 __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycles, float seed) {
@@ -107,6 +108,22 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
                 p[k] = __ffma2_rn(pr, rc, p[k]);
                 s2[k] = __ffma2_rn(pi, rc, s2[k]);
             }
+        } else if (MIX == FFMA2_FMUL) {
+            // does a scalar FP32 op cost one FMA-pipe cycle or two inside a packed stream?
+#pragma unroll
+            for (int k = 0; k < 6; ++k) {
+                p[k] = __ffma2_rn(p[k], b2, c2);
+                a[k] = a[k] * b;
+                s2[k] = __ffma2_rn(s2[k], b2, c2);
+            }
+        } else if (MIX == FFMA2_MUFU_INDEP) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                p[k] = __ffma2_rn(p[k], b2, c2);
+                a[k] = __int_as_float(__float_as_int(rcp_mufu(a[k])) ^ 1);
+                s2[k] = __ffma2_rn(s2[k], b2, c2);
+                p[k + 4] = __ffma2_rn(p[k + 4], b2, c2);
+            }
         } else if (MIX == DFMA) {
 #pragma unroll
             for (int k = 0; k < kChains; ++k) dd[k] = fma(dd[k], (double)b, (double)c);
@@ -129,12 +146,17 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
 }
 
 template <int MIX>
-void run(int sms, int ctas_per_sm, float* out, long long* cyc_dev, bool last) {
+void run(int sms, int ctas_req, float* out, long long* cyc_dev, bool last) {
+    // exactly one resident wave: every CTA runs concurrently for the whole kernel, so CTA 0's clock64() span is the
+    // kernel's span and instr/cycles is a true per-SMSP rate
+    int occ = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, bench_kernel<MIX>, 256, 0));
+    const int ctas_per_sm = occ < ctas_req ? occ : ctas_req;
     const int grid = sms * ctas_per_sm;
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);  // warm-up
+    for (int w = 0; w < 3; ++w) bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);  // warm-up (clock ramp)
     CK(cudaDeviceSynchronize());
     float best = 1e30f;
     long long cyc_best = 0;
@@ -149,13 +171,13 @@ void run(int sms, int ctas_per_sm, float* out, long long* cyc_dev, bool last) {
         CK(cudaMemcpy(&c0, cyc_dev, sizeof(c0), cudaMemcpyDeviceToHost));
         if (ms < best) { best = ms; cyc_best = c0; }
     }
-    // warp-instructions per clock per SMSP from the in-kernel cycle count of CTA 0
     const double warps_per_smsp = ctas_per_sm * 8 / 4.0;
     const double instr = (double)kIters * kInstr[MIX] * warps_per_smsp;
     const double ipc = instr / (double)cyc_best;
-    const double mhz = (double)cyc_best / (best * 1e-3) * 1e-6;
-    printf("  \"%s\": {\"ctas_per_sm\": %d, \"warp_instr_per_clk_per_smsp\": %.4f, \"cycles\": %lld, \"ms\": %.4f, \"sm_mhz_upper\": %.0f}%s\n",
-           kMixName[MIX], ctas_per_sm, ipc, cyc_best, best, mhz, last ? "" : ",");
+    const double mhz = (double)cyc_best / (best * 1e-3) * 1e-6;  // CTA 0 cycles / event time: the SM clock (slightly low)
+    printf("  \"%s\": {\"ctas_per_sm\": %d, \"warp_instr_per_clk_per_smsp\": %.4f, \"clk_per_warp_instr\": %.3f, "
+           "\"cycles\": %lld, \"ms\": %.4f, \"sm_mhz\": %.0f}%s\n",
+           kMixName[MIX], ctas_per_sm, ipc, 1.0 / ipc, cyc_best, best, mhz, last ? "" : ",");
     CK(cudaEventDestroy(e0));
     CK(cudaEventDestroy(e1));
 }
@@ -178,7 +200,9 @@ int main(int argc, char** argv) {
     run<KERNEL_MIX>(sms, ctas, out, cyc, false);
     run<PAIRED_MIX>(sms, ctas, out, cyc, false);
     run<DFMA>(sms, ctas, out, cyc, false);
-    run<LDS128>(sms, ctas, out, cyc, true);
+    run<LDS128>(sms, ctas, out, cyc, false);
+    run<FFMA2_FMUL>(sms, ctas, out, cyc, false);
+    run<FFMA2_MUFU_INDEP>(sms, ctas, out, cyc, true);
     printf("}\n");
     return 0;
 }

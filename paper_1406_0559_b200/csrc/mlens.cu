@@ -59,7 +59,7 @@ struct mlens {
     cudaEvent_t ev0, ev1, evk0, evk1;
     float last_ms, last_kernel_ms;
     // options
-    int opt_kernel, opt_binning, opt_ctas_per_sm;
+    int opt_kernel, opt_binning, opt_ctas_per_sm, opt_paired, opt_rays;
 };
 
 namespace {
@@ -85,6 +85,10 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     P.lens_raw = h->lens_dev;
     P.n_lens = (int)h->n_lens;
     P.rho2 = 0.25;  // rho = 0.5 sqrt(max(m,1))
+    {
+        const double hd = 0.5 * mlk::kTile * h->d * 1.4142135623730951;  // tile half-diagonal
+        P.rho2_tile = 4.0 * hd * hd;
+    }
     P.count = count; P.ray_y = ray_y; P.ray_pix = ray_pix;
     P.counters = h->counters_dev;
     P.bin_mode = h->opt_binning;
@@ -110,11 +114,22 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     }
     P.chunk = chunk; P.n_chunks = n_chunks;
     const size_t smem = sizeof(mlk::TileShared) + (size_t)chunk * 16 * (n_chunks > 1 ? 3 : 2);
-    MLENS_CUDA(cudaFuncSetAttribute(mlk::shoot_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
     long long grid = (long long)h->sm_count * h->opt_ctas_per_sm;
     if (grid > n_tiles) grid = n_tiles;
-    mlk::shoot_fp32_kernel<<<(unsigned)grid, mlk::kThreads, smem, st>>>(P);
+    void (*kern)(const mlk::ShootParams) = nullptr;
+    const int code = h->opt_rays * 100 + h->opt_paired;
+    switch (code) {
+#define MLENS_VARIANT(R, PAIRS) case R * 100 + PAIRS: kern = mlk::shoot_fp32_kernel<R, PAIRS>; break;
+        MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
+        MLENS_VARIANT(16, 6) MLENS_VARIANT(16, 8)
+        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2) MLENS_VARIANT(8, 4)
+#undef MLENS_VARIANT
+        default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d paired_rcp=%d", h->opt_rays, h->opt_paired);
+    }
+    const int threads = mlk::kTile * mlk::kTile / h->opt_rays;
+    MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<(unsigned)grid, threads, smem, st>>>(P);
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }
@@ -204,7 +219,7 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
     h->npix = npix; h->n_lens = n_lens; h->geo = g;
     h->device = dev; h->sm_count = prop.multiProcessorCount;
-    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2;
+    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2; h->opt_paired = 0; h->opt_rays = 8;
 
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
@@ -261,6 +276,12 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
     } else if (!strcmp(key, "ctas_per_sm")) {
         if (value < 1 || value > 8) return fail(MLENS_EINVAL, "ctas_per_sm must be 1..8");
         h->opt_ctas_per_sm = (int)value;
+    } else if (!strcmp(key, "paired_rcp")) {
+        if (value < 0 || value > 8) return fail(MLENS_EINVAL, "paired_rcp must be 0..8");
+        h->opt_paired = (int)value;
+    } else if (!strcmp(key, "rays_per_thread")) {
+        if (value != 8 && value != 16) return fail(MLENS_EINVAL, "rays_per_thread must be 8 or 16");
+        h->opt_rays = (int)value;
     } else {
         return fail(MLENS_EINVAL, "unknown option '%s'", key);
     }

@@ -20,12 +20,12 @@
 
 namespace mlk {
 
-constexpr int kThreads = 256;       // threads per CTA
 constexpr int kTile = 64;           // tile is kTile x kTile rays
-constexpr int kR = 16;              // rays per thread, consecutive along x1
+constexpr int kMaxThreads = 512;    // threads per CTA = kTile*kTile/kR (kR rays per thread, consecutive along x1)
 constexpr int kNearMax = 32;        // capacity of the per-tile near-lens list
 constexpr int kWin = 32;            // binning window side (pixels), BIN_WINDOW mode
-constexpr float kFar = 1.0e15f;     // offset of a neutralised main-list entry (contributes exactly 0)
+constexpr float kFar = 1.0e8f;      // offset of a neutralised main-list entry (c = 0: contributes exactly 0;
+                                    // r2^2 = 4e32 stays finite for the shared reciprocal)
 
 enum BinMode { BIN_PER_RAY = 0, BIN_RUNS = 1, BIN_WARP = 2, BIN_WINDOW = 3 };
 
@@ -45,6 +45,7 @@ struct ShootParams {
     int chunk;                      // lenses per shared-memory chunk (multiple of 4)
     int n_chunks;
     double rho2;                    // near-list radius^2 for m <= 1 (scaled by max(m,1))
+    double rho2_tile;               // and never less than (2 x tile half-diagonal)^2: |delta| << |zeta| must hold
     // outputs
     int* count;                     // npix*npix or nullptr
     double* ray_y;                  // optional per-ray outputs
@@ -111,7 +112,7 @@ __device__ __forceinline__ void warp_aggregated_add(int* count, int pix, int n, 
 // ---------------------------------------------------------------------------------------------------------------
 struct __align__(16) TileShared {
     uint64_t bar[2];                         // mbarriers of the raw-chunk double buffer
-    double part[kThreads / 32][2];           // per-warp partial sums of A_c
+    double part[kMaxThreads / 32][2];        // per-warp partial sums of A_c
     double near_zx[kNearMax], near_zy[kNearMax], near_m[kNearMax];
     int near_n;
     int win_ix0, win_iy0;                    // binning window origin (BIN_WINDOW)
@@ -136,7 +137,15 @@ __device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, 
     }
 }
 
-__global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootParams P) {
+// kPaired = number of the thread's kR/2 ray pairs per lens whose two reciprocals come from ONE MUFU.RCP:
+//   q = r2.x * r2.y;  t = rcp(q);  1/r2.x = t * r2.y;  1/r2.y = t * r2.x        (3 FMUL + 1 MUFU instead of 2 MUFU)
+// MUFU issues 4 lanes/clk/SMSP (8 clk per warp instruction) against 2 clk per FFMA2, so with kPaired = 0 the XU pipe
+// is the bound (16 clk per pair vs 12 on the FMA pipe); sharing reciprocals on part of the pairs balances the two
+// pipes (measured by alu_microbench.cu).
+template <int kR, int kPaired>
+__global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const ShootParams P) {
+    constexpr int kThreads = kTile * kTile / kR;
+    constexpr int kTx = kTile / kR;  // threads along x1
     extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
     TileShared& sh = *reinterpret_cast<TileShared*>(smem_raw_bytes);
     float4* xf = reinterpret_cast<float4*>(smem_raw_bytes + sizeof(TileShared));  // transformed chunk
@@ -144,7 +153,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
-    const int tx = tid & 3, ty = tid >> 2;  // 4 threads x 16 rays along x1, 64 rows along x2
+    const int tx = tid % kTx, ty = tid / kTx;  // kTx threads x kR rays along x1, 64 rows along x2
 
     if (tid == 0) {
         mbar_init(&sh.bar[0], 1);
@@ -201,7 +210,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
                     const float4 q = raw[t];
                     const double zx = Zcx - (double)q.x, zy = Zcy - (double)q.y, m = (double)q.z;
                     const double r2 = zx * zx + zy * zy;
-                    bool near = r2 < P.rho2 * fmax(m, 1.0);
+                    bool near = r2 < fmax(P.rho2 * fmax(m, 1.0), P.rho2_tile);
                     if (near) {
                         const int slot = atomicAdd(&sh.near_n, 1);
                         if (slot < kNearMax) {
@@ -243,9 +252,11 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
             for (int w = 0; w < kThreads / 32; ++w) { Acr += sh.part[w][0]; Aci += sh.part[w][1]; }
 
             // (4) HOT LOOP: all lenses of the chunk x this thread's kR rays
+            float4 qn = xf[0];
 #pragma unroll 2
             for (int l = 0; l < n_pad; ++l) {
-                const float4 q = xf[l];  // broadcast LDS.128: (zeta_x, zeta_y, c_r, c_i)
+                const float4 q = qn;  // (zeta_x, zeta_y, c_r, c_i)
+                qn = xf[l + 1];       // broadcast LDS.128 one lens ahead (xf[n_pad] is readable: raw0 follows xf)
                 const float dy = dyf + q.y;
                 const float dy2 = dy * dy;
                 const float a = q.w * dy;    //  c_i * dy
@@ -257,7 +268,13 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
                 for (int j = 0; j < kR / 2; ++j) {
                     const float2 dx = __fadd2_rn(dxb[j], NX);
                     const float2 r2 = __ffma2_rn(dx, dx, DY2);
-                    const float2 rc = make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y));
+                    float2 rc;
+                    if (j < kPaired) {
+                        const float t = rcp_mufu(r2.x * r2.y);
+                        rc = make_float2(t * r2.y, t * r2.x);
+                    } else {
+                        rc = make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y));
+                    }
                     const float2 pr = __ffma2_rn(CR, dx, AA);
                     const float2 pi = __ffma2_rn(CI, dx, BB);
                     Sr[j] = __ffma2_rn(pr, rc, Sr[j]);
@@ -269,6 +286,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
 
         // (5) per-ray FP64 epilogue: alpha, Eq. (1), pixel id; (6) binning
         const int n_near = min(sh.near_n, kNearMax);
+        const bool near_overflow = sh.near_n > kNearMax;
         const long long jray = tj0 + ty;
         const bool row_ok = jray < P.j0 + P.nj;
         const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
@@ -307,6 +325,18 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_fp32_kernel(const ShootPara
                 al2 += f * wy;
             }
             const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
+            if (near_overflow) {
+                // more than kNearMax lenses within rho of this tile: the FP32 list then holds lenses it cannot sum
+                // accurately (or at all: r2 = 0), so the tile's rays take Eq. (1) in plain FP64 from global memory
+                al1 = al2 = 0.0;
+                for (int q = 0; q < P.n_lens; ++q) {
+                    const float4 l = __ldg(P.lens_raw + q);
+                    const double wx = x1 - (double)l.x, wy = x2 - (double)l.y;
+                    const double f = (double)l.z / (wx * wx + wy * wy);
+                    al1 += f * wx;
+                    al2 += f * wy;
+                }
+            }
             const double y1 = P.f1 * x1 - al1;
             const double y2 = P.f2 * x2 - al2;
             int pix;

@@ -181,6 +181,39 @@ def test_binning_variants_and_fp64_kernel_agree(ml, oracle):
     assert np.abs(maps[1][0].astype(np.int64) - ref["count"]).sum() <= TOL_L1 * in_map
 
 
+@pytest.mark.parametrize("paired", [0, 1, 2, 3, 4])
+def test_paired_reciprocal_variants_meet_the_tolerances(ml, oracle, paired):
+    # "paired_rcp": k of a thread's 8 ray pairs per lens share one MUFU reciprocal; every setting must hold P10
+    cfg = fields.CONFIGS[4]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        h.set_option("paired_rcp", paired)
+        g = h.geometry
+        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 17, 3, 3, 0, size=192)
+        tot = {"in_map": 0, "l1": 0}
+        for b in blocks:
+            r = check_block(ml, oracle, h, cfg, xy, m, b)
+            tot["in_map"] += r["in_map"]; tot["l1"] += r["l1"]
+    assert tot["l1"] <= max(2, TOL_L1 * tot["in_map"]), tot
+
+
+def test_near_list_overflow_falls_back_to_fp64(ml, oracle):
+    # more lenses within rho of one tile than the near list holds (32): those tiles take Eq. 1 in plain FP64
+    L, npix, sub = 4.0, 64, 4
+    d = L / npix / sub
+    u = fields.uniform01(99, 0, 2 * 60)
+    cluster = np.stack([0.3 * (u[0::2] - 0.5), 0.3 * (u[1::2] - 0.5)], axis=1)  # 60 lenses inside a 0.3 x 0.3 box
+    far, _ = fields.random_field(20, 6.0, 98)
+    xy = np.concatenate([cluster.astype(np.float32), far])
+    m = np.full((len(xy),), 0.05, np.float32)
+    cfg = fields.MapConfig("overflow", npix, L, 0.2, 0.05, 0.0, sub, "unit", 0)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        g = h.geometry
+        for b in [(g.n1 // 2 - 96, g.n2 // 2 - 96, 192, 192), (0, 0, 130, 70)]:
+            r = check_block(ml, oracle, h, cfg, xy, m, b)
+            assert r["l1"] <= max(2, 2 * r["mismatch"]) and r["mismatch"] <= 2
+
+
 def test_mirror_symmetry_on_gpu(ml):
     # P6 through the CUDA path
     cfg = dataclasses.replace(fields.CONFIGS[1], npix=128, sub=6)
