@@ -123,7 +123,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
 #define MLENS_VARIANT(R, PAIRS) case R * 100 + PAIRS: kern = mlk::shoot_fp32_kernel<R, PAIRS>; break;
         MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
         MLENS_VARIANT(16, 6) MLENS_VARIANT(16, 8)
-        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2) MLENS_VARIANT(8, 4)
+        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2) MLENS_VARIANT(8, 3) MLENS_VARIANT(8, 4)
 #undef MLENS_VARIANT
         default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d paired_rcp=%d", h->opt_rays, h->opt_paired);
     }
