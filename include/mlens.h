@@ -111,8 +111,8 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream);
  *   "binning"   0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
  *               3 = + CTA-private shared-memory window
  *   "ctas_per_sm"  persistent CTAs per SM (default 2)
- *   "paired_rcp"   how many of a thread's ray pairs per lens share ONE MUFU reciprocal (default 0 = one MUFU.RCP per
- *                  interaction)
+ *   "shared_rcp"   how many of a thread's 4-ray groups per lens take their four reciprocals from TWO MUFU.RCP of packed
+ *                  products (0 = one MUFU.RCP per interaction); at most rays_per_thread/4
  *   "rays_per_thread"  8 (512-thread CTAs, default) or 16 (256-thread CTAs); the tile is 64 x 64 rays either way
  * Returns MLENS_EINVAL for an unknown key or value. */
 int mlens_set_option(mlens_t* h, const char* key, long long value);

@@ -59,7 +59,7 @@ struct mlens {
     cudaEvent_t ev0, ev1, evk0, evk1;
     float last_ms, last_kernel_ms;
     // options
-    int opt_kernel, opt_binning, opt_ctas_per_sm, opt_paired, opt_rays;
+    int opt_kernel, opt_binning, opt_ctas_per_sm, opt_shared, opt_rays;
 };
 
 namespace {
@@ -118,14 +118,13 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     long long grid = (long long)h->sm_count * h->opt_ctas_per_sm;
     if (grid > n_tiles) grid = n_tiles;
     void (*kern)(const mlk::ShootParams) = nullptr;
-    const int code = h->opt_rays * 100 + h->opt_paired;
+    const int code = h->opt_rays * 100 + h->opt_shared;
     switch (code) {
-#define MLENS_VARIANT(R, PAIRS) case R * 100 + PAIRS: kern = mlk::shoot_fp32_kernel<R, PAIRS>; break;
+#define MLENS_VARIANT(R, SH) case R * 100 + SH: kern = mlk::shoot_fp32_kernel<R, SH>; break;
         MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
-        MLENS_VARIANT(16, 6) MLENS_VARIANT(16, 8)
-        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2) MLENS_VARIANT(8, 3) MLENS_VARIANT(8, 4)
+        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2)
 #undef MLENS_VARIANT
-        default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d paired_rcp=%d", h->opt_rays, h->opt_paired);
+        default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d shared_rcp=%d", h->opt_rays, h->opt_shared);
     }
     const int threads = mlk::kTile * mlk::kTile / h->opt_rays;
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -219,7 +218,7 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
     h->npix = npix; h->n_lens = n_lens; h->geo = g;
     h->device = dev; h->sm_count = prop.multiProcessorCount;
-    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2; h->opt_paired = 0; h->opt_rays = 8;
+    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2; h->opt_shared = 0; h->opt_rays = 8;
 
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
@@ -276,9 +275,9 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
     } else if (!strcmp(key, "ctas_per_sm")) {
         if (value < 1 || value > 8) return fail(MLENS_EINVAL, "ctas_per_sm must be 1..8");
         h->opt_ctas_per_sm = (int)value;
-    } else if (!strcmp(key, "paired_rcp")) {
-        if (value < 0 || value > 8) return fail(MLENS_EINVAL, "paired_rcp must be 0..8");
-        h->opt_paired = (int)value;
+    } else if (!strcmp(key, "shared_rcp")) {
+        if (value < 0 || value > 4) return fail(MLENS_EINVAL, "shared_rcp must be 0..4");
+        h->opt_shared = (int)value;
     } else if (!strcmp(key, "rays_per_thread")) {
         if (value != 8 && value != 16) return fail(MLENS_EINVAL, "rays_per_thread must be 8 or 16");
         h->opt_rays = (int)value;

@@ -137,12 +137,13 @@ __device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, 
     }
 }
 
-// kPaired = number of the thread's kR/2 ray pairs per lens whose two reciprocals come from ONE MUFU.RCP:
-//   q = r2.x * r2.y;  t = rcp(q);  1/r2.x = t * r2.y;  1/r2.y = t * r2.x        (3 FMUL + 1 MUFU instead of 2 MUFU)
-// MUFU issues 4 lanes/clk/SMSP (8 clk per warp instruction) against 2 clk per FFMA2, so with kPaired = 0 the XU pipe
-// is the bound (16 clk per pair vs 12 on the FMA pipe); sharing reciprocals on part of the pairs balances the two
-// pipes (measured by alu_microbench.cu).
-template <int kR, int kPaired>
+// kShared = number of the thread's 4-ray groups (two packed ray pairs A, B) per lens whose four reciprocals come from
+// TWO MUFU.RCP instead of four, with packed multiplies only:
+//   q = r2A * r2B (FMUL2);  t = (rcp q.x, rcp q.y);  1/r2A = t * r2B (FMUL2);  1/r2B = t * r2A (FMUL2)
+// Kept as an ablation switch only: measured on B200 it LOSES (150.7 -> 159.2 -> 175.8 ms for 0/1/2 shared groups,
+// profiles/r1_summary.md).  Packed FP32 instructions with three distinct register-pair operands are bound by
+// register-file read bandwidth (3.0 clk, not 2.0), so the three extra FMUL2 cost more than the two MUFU they save.
+template <int kR, int kShared>
 __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const ShootParams P) {
     constexpr int kThreads = kTile * kTile / kR;
     constexpr int kTx = kTile / kR;  // threads along x1
@@ -253,7 +254,7 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
 
             // (4) HOT LOOP: all lenses of the chunk x this thread's kR rays
             float4 qn = xf[0];
-#pragma unroll 2
+#pragma unroll 4
             for (int l = 0; l < n_pad; ++l) {
                 const float4 q = qn;  // (zeta_x, zeta_y, c_r, c_i)
                 qn = xf[l + 1];       // broadcast LDS.128 one lens ahead (xf[n_pad] is readable: raw0 follows xf)
@@ -264,21 +265,30 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
                 const float2 NX = make_float2(q.x, q.x), DY2 = make_float2(dy2, dy2);
                 const float2 AA = make_float2(a, a), BB = make_float2(b, b);
                 const float2 CR = make_float2(q.z, q.z), CI = make_float2(q.w, q.w);
+float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
 #pragma unroll
                 for (int j = 0; j < kR / 2; ++j) {
-                    const float2 dx = __fadd2_rn(dxb[j], NX);
-                    const float2 r2 = __ffma2_rn(dx, dx, DY2);
-                    float2 rc;
-                    if (j < kPaired) {
-                        const float t = rcp_mufu(r2.x * r2.y);
-                        rc = make_float2(t * r2.y, t * r2.x);
+                    dx[j] = __fadd2_rn(dxb[j], NX);
+                    r2[j] = __ffma2_rn(dx[j], dx[j], DY2);
+                }
+#pragma unroll
+                for (int j = 0; j < kR / 2; j += 2) {
+                    if (j / 2 < kShared) {
+                        const float2 qq = __fmul2_rn(r2[j], r2[j + 1]);
+                        const float2 t = make_float2(rcp_mufu(qq.x), rcp_mufu(qq.y));
+                        rc[j] = __fmul2_rn(t, r2[j + 1]);
+                        rc[j + 1] = __fmul2_rn(t, r2[j]);
                     } else {
-                        rc = make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y));
+                        rc[j] = make_float2(rcp_mufu(r2[j].x), rcp_mufu(r2[j].y));
+                        rc[j + 1] = make_float2(rcp_mufu(r2[j + 1].x), rcp_mufu(r2[j + 1].y));
                     }
-                    const float2 pr = __ffma2_rn(CR, dx, AA);
-                    const float2 pi = __ffma2_rn(CI, dx, BB);
-                    Sr[j] = __ffma2_rn(pr, rc, Sr[j]);
-                    Si[j] = __ffma2_rn(pi, rc, Si[j]);
+                }
+#pragma unroll
+                for (int j = 0; j < kR / 2; ++j) {
+                    const float2 pr = __ffma2_rn(CR, dx[j], AA);
+                    const float2 pi = __ffma2_rn(CI, dx[j], BB);
+                    Sr[j] = __ffma2_rn(pr, rc[j], Sr[j]);
+                    Si[j] = __ffma2_rn(pi, rc[j], Si[j]);
                 }
             }
             __syncthreads();  // xf (and sh.part) may be overwritten by the next chunk / tile

@@ -181,13 +181,14 @@ def test_binning_variants_and_fp64_kernel_agree(ml, oracle):
     assert np.abs(maps[1][0].astype(np.int64) - ref["count"]).sum() <= TOL_L1 * in_map
 
 
-@pytest.mark.parametrize("paired", [0, 1, 2, 3, 4])
-def test_paired_reciprocal_variants_meet_the_tolerances(ml, oracle, paired):
-    # "paired_rcp": k of a thread's 8 ray pairs per lens share one MUFU reciprocal; every setting must hold P10
+@pytest.mark.parametrize("rays,shared", [(8, 0), (8, 1), (8, 2), (16, 0), (16, 1), (16, 2), (16, 4)])
+def test_shared_reciprocal_variants_meet_the_tolerances(ml, oracle, rays, shared):
+    # "shared_rcp": k of a thread's 4-ray groups per lens take 4 reciprocals from 2 MUFU.RCP; every setting must hold P10
     cfg = fields.CONFIGS[4]
     xy, m = fields.lens_field(cfg)
     with ml.Mlens.from_config(cfg, xy, m) as h:
-        h.set_option("paired_rcp", paired)
+        h.set_option("rays_per_thread", rays)
+        h.set_option("shared_rcp", shared)
         g = h.geometry
         blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 17, 3, 3, 0, size=192)
         tot = {"in_map": 0, "l1": 0}
