@@ -184,7 +184,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from paper_1406_0559_b200 import mlens
+    from paper_1406_0559_b200 import mlens, sharded
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -205,7 +205,9 @@ def run_ours(args):
     import dataclasses
 
     cfg0 = fields.CONFIGS[args.config]
-    cfg = dataclasses.replace(cfg0, seed=cfg0.seed + rank)  # weak scaling: an independent map per rank
+    shard = bool(args.shard) and world > 1
+    # default N > 1: weak scaling, an independent map per rank (the paper's way); --shard: ONE map, row bands per rank
+    cfg = cfg0 if shard else dataclasses.replace(cfg0, seed=cfg0.seed + rank)
     xy, m = fields.lens_field(cfg)
     n_lens = len(m)
     h = mlens.Mlens.from_config(cfg, xy, m)
@@ -218,6 +220,14 @@ def run_ours(args):
 
     def step(sync_stats=False):
         flush.fill_(1)  # evict the count map and lens list from L2 between steps
+        if shard:
+            t0k, t1k = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0k.record()
+            st_ = sharded.shoot_sharded(h, rank, world, count=count, mag=mag)[2]
+            t1k.record()
+            torch.cuda.synchronize()
+            st_["kernel_ms"] = t0k.elapsed_time(t1k)  # band kernel + all-reduce + Eq. 4
+            return st_
         return h.shoot(count=count, mag=mag, sync=sync_stats)[2]
 
     for _ in range(args.warmup):
@@ -251,7 +261,11 @@ def run_ours(args):
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         with mlens.Mlens.from_config(cfg, xy, m) as h2:
-            c_host, m_host, st2 = h2.shoot_host()
+            if shard:
+                c_dev, m_dev, st2 = sharded.shoot_sharded(h2, rank, world)
+                c_host, m_host = c_dev.cpu().numpy(), m_dev.cpu().numpy()
+            else:
+                c_host, m_host, st2 = h2.shoot_host()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -266,23 +280,29 @@ def run_ours(args):
         f_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         peak = sms * FP32_LANES_PER_SM * 2 * f_max_mhz * 1e6 / 1e12  # TFLOP/s at the maximum SM clock
         fpi = flops_per_interaction(cfg)
-        achieved = fpi * inter / (kern_ms * 1e-3) / 1e12
-        value = world * inter * args.steps / (ms_total * 1e-3)
+        # shard mode: each rank's kernel covers 1/world of the interactions (kern_ms then also holds the all-reduce)
+        achieved = fpi * (inter / (world if shard else 1)) / (kern_ms * 1e-3) / 1e12
+        maps = 1 if shard else world
+        value = maps * inter * args.steps / (ms_total * 1e-3)
+        # DRAM bytes of one shoot_fp32_kernel launch of the default workload (config 4, whole lattice), from
+        # profiles/r1_traffic_cfg4_full.csv (dram__bytes_read.sum + dram__bytes_write.sum); other workloads: not captured
+        traffic = 5098752 + 806948096 if (args.config == 4 and not shard) else None
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+            "ms_per_step": ms_total / max(1, args.steps), "higher_is_better": True, "scaling": "strong" if shard else "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(args.config, cfg0, n_lens, g.n1, g.n2), "rays_per_map": rays,
                        "interactions_per_map": inter, "rays_in_map": in_map,
                        "l2": "256 MiB device write between steps (inputs are smaller than L2)",
-                       "parallelism": f"{world} independent map(s), one per GPU (seed + rank)"},
-            "rays_per_s": world * rays * args.steps / (ms_total * 1e-3),
+                       "parallelism": (f"one map, {world} row bands + one int32 all-reduce" if shard else
+                                       f"{world} independent map(s), one per GPU (seed + rank)")},
+            "rays_per_s": maps * rays * args.steps / (ms_total * 1e-3),
             "clocks": clocks,
-            "e2e": {"value": world * inter * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
+            "e2e": {"value": maps * inter * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
                     "h2d_bytes_per_step": int(xy.nbytes + m.nbytes), "d2h_bytes_per_step": int(c_host.nbytes + m_host.nbytes)},
             "gpu_launches": 2 * args.steps,  # shoot_fp32_kernel + magnification_kernel per step (memsets are driver ops)
             "roofline": {"bound": "alu", "kernel": "shoot_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": None, "flops_per_interaction": fpi,
+                         "frac": achieved / peak, "traffic": traffic, "flops_per_interaction": fpi,
                          "kernel_ms": kern_ms,
                          "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 x {f_max_mhz:.0f} MHz (clocks.max.sm); "
                                         "no FP32 figure in MEASURED_PEAKS.json",
@@ -340,6 +360,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=sorted(fields.CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard", action="store_true", help="N > 1: shoot ONE map in row bands + one all-reduce (strong scaling)")
     ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
     args = ap.parse_args()

@@ -58,6 +58,15 @@ typedef struct {
     double kappa_s, kappa_star, n_avg; /* Eq. 2 split; N_avg = (p/d)^2 */
 } mlens_geometry;
 
+typedef struct {
+    long long n_pixels;    /* npix*npix */
+    long long sum_count;   /* sum of all pixel counts (= rays_in_map of the map's own shoot) */
+    long long n_clamped;   /* pixels with count >= n_bins-1: they all sit in the last bin of the histogram */
+    int min_count, max_count;
+    double mean_count;     /* <N>  = sum_count / n_pixels           (mapmeta.dat) */
+    double mean_mu;        /* <mu> = <N> / N_avg                    (Eq. 4) */
+} mlens_map_stats;
+
 /* Create a map context (a map is defined by kappa, gamma, s, width, resolution, N_avg and the
  * lens positions/masses).
  *   kappa, gamma, s    total convergence, shear, smooth-matter fraction (0 <= s <= 1)
@@ -97,6 +106,20 @@ int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* 
 /* Step a5 alone (Eq. 4): mag = (float)((double)count / N_avg); also refreshes max_count.  Asynchronous. */
 int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* cuda_stream);
 
+/* Map statistics.  The full magnification probability distribution of PAPER.md:307 ("the
+ * frequency of each magnification value in a map is counted and then divided by the total number of pixels"): since
+ * mu = count/N_avg with integer counts, the MPD is the histogram of the counts, hist[c] = number of pixels whose count
+ * is c (divide by n_pixels for the probability, c by N_avg for the magnification axis).  Also <N> and <mu>
+ * (mapmeta.dat).
+ *   count_dev  DEVICE npix*npix int32 (a finished count map)
+ *   hist_dev   DEVICE n_bins unsigned 64-bit integers, caller-owned; ZEROED by the call, then filled.  Counts
+ *              >= n_bins-1 are clamped into the last bin (use n_bins >= max_count+2 for the unclamped MPD)
+ *   n_bins     >= 2
+ *   stats      HOST or NULL.  NULL: asynchronous on `cuda_stream`.  Non-NULL: synchronises the stream and fills it.
+ * Integer arithmetic only: the result is exact.  MLENS_EINVAL for NULL pointers or n_bins < 2. */
+int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, int n_bins, void* cuda_stream,
+              mlens_map_stats* stats);
+
 /* Derived lattice and parameters (pure host data; valid from mlens_create on). */
 int mlens_get_geometry(const mlens_t* h, mlens_geometry* g);
 
@@ -107,7 +130,8 @@ int mlens_get_stats(mlens_t* h, void* cuda_stream, mlens_stats* stats);
 int mlens_reset_stats(mlens_t* h, void* cuda_stream);
 
 /* Tuning / ablation switches.  Keys:
- *   "kernel"    0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 1 = FP32 difference-form kernel (default)
+ *   "kernel"    0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 1 = FP32 difference-form kernel (default),
+ *               2 = ABLATION: plain-form FP32 kernel (does NOT meet the parity tolerances; <= 12000 lenses)
  *   "binning"   0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
  *               3 = + CTA-private shared-memory window
  *   "ctas_per_sm"  persistent CTAs per SM (default 2)

@@ -142,3 +142,16 @@ def magnification(count, n_avg):
     lib().oracle_magnification(_p(c, ctypes.c_int), ctypes.c_longlong(c.size), ctypes.c_double(n_avg),
                                _p(mag, ctypes.c_float))
     return mag
+
+
+def mpd(count, n_bins, n_avg):
+    """Full MPD as the histogram of the integer counts + map means.  Returns
+    (hist uint64 [n_bins], dict(n_pixels, sum_count, n_clamped, min_count, max_count, mean_count, mean_mu))."""
+    c = np.ascontiguousarray(count, dtype=np.int32).reshape(-1)
+    hist = np.empty((int(n_bins),), dtype=np.uint64)
+    out = np.zeros((4,), dtype=np.int64)
+    lib().oracle_mpd(_p(c, ctypes.c_int), ctypes.c_longlong(c.size), _p(hist, ctypes.c_ulonglong), ctypes.c_int(int(n_bins)),
+                     _p(out, ctypes.c_longlong))
+    mean = float(out[0]) / float(c.size)
+    return hist, {"n_pixels": int(c.size), "sum_count": int(out[0]), "n_clamped": int(out[1]), "min_count": int(out[2]),
+                  "max_count": int(out[3]), "mean_count": mean, "mean_mu": mean / float(n_avg)}

@@ -196,6 +196,26 @@ void oracle_magnification(const int* count, long long n_pixels, double n_avg, fl
     for (long long q = 0; q < n_pixels; ++q) mag[q] = (float)((double)count[q] / n_avg);
 }
 
+// Full magnification probability distribution ("the frequency of each magnification value in a map is
+// counted and then divided by the total number of pixels") and the map means of mapmeta.dat.  mu is
+// count/N_avg (Eq. 4) with integer counts, so the MPD is the histogram of the counts: hist[c] = #pixels with count c.
+// Counts >= n_bins-1 are put in the last bin (same clamping convention as include/mlens.h).  One pixel at a time.
+// out[0] = sum of counts, out[1] = number of clamped pixels, out[2] = min count, out[3] = max count.
+void oracle_mpd(const int* count, long long n_pixels, unsigned long long* hist, int n_bins, long long* out) {
+    for (int b = 0; b < n_bins; ++b) hist[b] = 0ull;
+    long long sum = 0, clamped = 0, cmin = 2147483647LL, cmax = 0;
+    for (long long q = 0; q < n_pixels; ++q) {
+        const int c = count[q];
+        sum += c;
+        if (c < cmin) cmin = c;
+        if (c > cmax) cmax = c;
+        int b = c < 0 ? 0 : c;
+        if (b >= n_bins - 1) { b = n_bins - 1; ++clamped; }
+        hist[b] += 1ull;
+    }
+    out[0] = sum; out[1] = clamped; out[2] = cmin; out[3] = cmax;
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

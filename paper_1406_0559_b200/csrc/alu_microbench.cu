@@ -24,6 +24,7 @@
 
 constexpr int kIters = 16384;
 constexpr int kChains = 16;
+static double g_clock_hz = 1.965e9;  // set from cudaDeviceProp::clockRate (the maximum SM clock) in main()
 
 __device__ __forceinline__ float rcp_mufu(float x) {
     float r;
@@ -31,15 +32,17 @@ __device__ __forceinline__ float rcp_mufu(float x) {
     return r;
 }
 
-enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, FFMA2_FMUL, FFMA2_MUFU_INDEP, N_MIX };
+enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, FFMA2_FMUL, FFMA2_MUFU_INDEP, FFMA2_3PAIRS, FFMA2_UBCAST, FFMA_3REGS, SHARED_MIX, N_MIX };
 static const char* kMixName[N_MIX] = {"ffma", "ffma2", "mufu_rcp", "ffma4_mufu1", "kernel_mix_6ffma2_2mufu",
                                       "paired_mix_6ffma2_3fmul_1mufu", "dfma", "fadd2", "lds128_broadcast",
-                                      "ffma2x12_fmulx6", "ffma2x12_mufux4_independent"};
+                                      "ffma2x12_fmulx6", "ffma2x12_mufux4_independent",
+                                      "ffma2_three_distinct_pairs", "ffma2_uniform_bcast_operand", "ffma_three_distinct_regs",
+                                      "shared_mix_12ffma2_3fmul2_2mufu_per_4rays"};
 // warp-instructions issued per inner iteration per thread, FP32 flops per iteration per thread
-static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains, 18, 16};
+static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains, 18, 16, kChains, kChains, kChains, 68};
 
 template <int MIX>
-__global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycles, float seed) {
+__global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycles, float seed, float useed) {
     __shared__ float4 sm[256];
     sm[threadIdx.x] = make_float4(seed, seed * 0.5f, seed * 0.25f, 1.0f);
     __syncthreads();
@@ -55,6 +58,16 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
     for (int k = 0; k < kChains / 2; ++k) { p[k] = make_float2(a[2 * k], a[2 * k + 1]); s2[k] = make_float2(0.f, 0.f); }
     const float b = 0.999f + seed * 1e-6f, c = seed * 1e-3f;
     const float2 b2 = make_float2(b, b), c2 = make_float2(c, c);
+    float2 xx[kChains / 2], yy[kChains / 2];
+    float xs[kChains], ys[kChains];
+#pragma unroll
+    for (int k = 0; k < kChains / 2; ++k) {
+        xx[k] = make_float2(seed + 0.01f * (float)(k + threadIdx.x), seed - 0.02f * k);
+        yy[k] = make_float2(0.5f * seed + 0.003f * (float)(threadIdx.x - k), 1.f + 1e-3f * k);
+    }
+#pragma unroll
+    for (int k = 0; k < kChains; ++k) { xs[k] = xx[k >> 1].x + k; ys[k] = yy[k >> 1].y - k; }
+    const float2 u2 = make_float2(useed, useed);  // kernel parameter: lives in a uniform register
     const long long t0 = clock64();
     for (int it = 0; it < kIters; ++it) {
         if (MIX == FFMA) {
@@ -124,6 +137,34 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
                 s2[k] = __ffma2_rn(s2[k], b2, c2);
                 p[k + 4] = __ffma2_rn(p[k + 4], b2, c2);
             }
+        } else if (MIX == FFMA2_3PAIRS) {
+            // accumulate form S += X*Y: three distinct register pairs per instruction (register-file read bound)
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) s2[k] = __ffma2_rn(xx[k], yy[(k + r) & (kChains / 2 - 1)], s2[k]);
+        } else if (MIX == FFMA2_UBCAST) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) s2[k] = __ffma2_rn(u2, xx[(k + r) & (kChains / 2 - 1)], s2[k]);
+        } else if (MIX == FFMA_3REGS) {
+#pragma unroll
+            for (int k = 0; k < kChains; ++k) a[k] = fmaf(xs[k], ys[k], a[k]);
+        } else if (MIX == SHARED_MIX) {
+            // the shared_rcp group: 4 rays (pairs A, B) take 4 reciprocals from 2 MUFU + 3 FMUL2
+#pragma unroll
+            for (int k = 0; k < kChains / 2; k += 2) {
+                const float2 dxa = __fadd2_rn(p[k], c2), dxc = __fadd2_rn(p[k + 1], c2);
+                const float2 ra = __ffma2_rn(dxa, dxa, b2), rb = __ffma2_rn(dxc, dxc, b2);
+                const float2 qq = __fmul2_rn(ra, rb);
+                const float2 t = make_float2(rcp_mufu(qq.x), rcp_mufu(qq.y));
+                const float2 rca = __fmul2_rn(t, rb), rcb = __fmul2_rn(t, ra);
+                p[k] = __ffma2_rn(__ffma2_rn(b2, dxa, c2), rca, p[k]);
+                s2[k] = __ffma2_rn(__ffma2_rn(c2, dxa, b2), rca, s2[k]);
+                p[k + 1] = __ffma2_rn(__ffma2_rn(b2, dxc, c2), rcb, p[k + 1]);
+                s2[k + 1] = __ffma2_rn(__ffma2_rn(c2, dxc, b2), rcb, s2[k + 1]);
+            }
         } else if (MIX == DFMA) {
 #pragma unroll
             for (int k = 0; k < kChains; ++k) dd[k] = fma(dd[k], (double)b, (double)c);
@@ -140,7 +181,7 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
 #pragma unroll
     for (int k = 0; k < kChains; ++k) s += a[k] + (float)dd[k];
 #pragma unroll
-    for (int k = 0; k < kChains / 2; ++k) s += p[k].x + p[k].y + s2[k].x + s2[k].y;
+    for (int k = 0; k < kChains / 2; ++k) s += p[k].x + p[k].y + s2[k].x + s2[k].y + xx[k].x + yy[k].y;
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
     if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
@@ -156,13 +197,13 @@ void run(int sms, int ctas_req, float* out, long long* cyc_dev, bool last) {
     cudaEvent_t e0, e1;
     CK(cudaEventCreate(&e0));
     CK(cudaEventCreate(&e1));
-    for (int w = 0; w < 3; ++w) bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);  // warm-up (clock ramp)
+    for (int w = 0; w < 3; ++w) bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f, 0.5f);  // warm-up (clock ramp)
     CK(cudaDeviceSynchronize());
     float best = 1e30f;
     long long cyc_best = 0;
     for (int rep = 0; rep < 5; ++rep) {
         CK(cudaEventRecord(e0));
-        bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f);
+        bench_kernel<MIX><<<grid, 256>>>(out, cyc_dev, 1.0f, 0.5f);
         CK(cudaEventRecord(e1));
         CK(cudaEventSynchronize(e1));
         float ms;
@@ -171,15 +212,60 @@ void run(int sms, int ctas_req, float* out, long long* cyc_dev, bool last) {
         CK(cudaMemcpy(&c0, cyc_dev, sizeof(c0), cudaMemcpyDeviceToHost));
         if (ms < best) { best = ms; cyc_best = c0; }
     }
+    // Throughput = total work / total (event) time.  CTA 0's own clock64() span must NOT be used: the warp scheduler
+    // favours the oldest warps, so co-resident CTAs finish one after another (CTA 0 of 4 ends after 1/4 of the
+    // kernel) and its span overstates the per-SMSP rate by up to the number of resident CTAs.
     const double warps_per_smsp = ctas_per_sm * 8 / 4.0;
     const double instr = (double)kIters * kInstr[MIX] * warps_per_smsp;
-    const double ipc = instr / (double)cyc_best;
-    const double mhz = (double)cyc_best / (best * 1e-3) * 1e-6;  // CTA 0 cycles / event time: the SM clock (slightly low)
+    const double clk = best * 1e-3 * g_clock_hz;  // SM cycles of the whole launch at the maximum SM clock
+    const double ipc = instr / clk;
     printf("  \"%s\": {\"ctas_per_sm\": %d, \"warp_instr_per_clk_per_smsp\": %.4f, \"clk_per_warp_instr\": %.3f, "
-           "\"cycles\": %lld, \"ms\": %.4f, \"sm_mhz\": %.0f}%s\n",
-           kMixName[MIX], ctas_per_sm, ipc, 1.0 / ipc, cyc_best, best, mhz, last ? "" : ",");
+           "\"cta0_cycles\": %lld, \"ms\": %.4f}%s\n",
+           kMixName[MIX], ctas_per_sm, ipc, 1.0 / ipc, cyc_best, best, last ? "" : ",");
     CK(cudaEventDestroy(e0));
     CK(cudaEventDestroy(e1));
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// binning sub-roof: throughput of integer REDs into an int32 map, by address pattern
+//   0 random over the whole map   1 one address per warp (32-way same address)   2 neighbouring addresses (coalesced)
+//   3 random within a 32x32 window per CTA (the footprint of a 64x64-ray tile, App. A.3)
+// ---------------------------------------------------------------------------------------------------------------
+template <int PATTERN>
+__global__ void __launch_bounds__(256) red_kernel(int* map, unsigned n_pix_mask, int reps) {
+    unsigned x = (blockIdx.x * 256u + threadIdx.x) * 2654435761u + 12345u;
+    const unsigned win = (blockIdx.x * 40503u) & n_pix_mask;
+    for (int r = 0; r < reps; ++r) {
+        x = x * 1664525u + 1013904223u;  // LCG
+        unsigned a;
+        if (PATTERN == 0) a = (x >> 4) & n_pix_mask;
+        else if (PATTERN == 1) a = (((blockIdx.x * 8u + (threadIdx.x >> 5)) * 977u + r) * 64u) & n_pix_mask;
+        else if (PATTERN == 2) a = ((blockIdx.x * 256u + threadIdx.x) + (unsigned)r * 65536u) & n_pix_mask;
+        else a = (win + ((x >> 8) & 1023u)) & n_pix_mask;
+        atomicAdd(map + a, 1);  // result unused -> RED.E.ADD
+    }
+}
+
+template <int PATTERN>
+void run_red(const char* name, int sms, int* map, unsigned mask, bool last) {
+    const int reps = 2048, grid = sms * 8;
+    red_kernel<PATTERN><<<grid, 256>>>(map, mask, 64);
+    CK(cudaDeviceSynchronize());
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        CK(cudaEventRecord(e0));
+        red_kernel<PATTERN><<<grid, 256>>>(map, mask, reps);
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        float ms;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        if (ms < best) best = ms;
+    }
+    printf("  \"%s\": {\"reds_per_s\": %.4e, \"ms\": %.4f}%s\n", name, (double)grid * 256 * reps / (best * 1e-3), best,
+           last ? "" : ",");
 }
 
 int main(int argc, char** argv) {
@@ -187,6 +273,7 @@ int main(int argc, char** argv) {
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, 0));
     const int sms = prop.multiProcessorCount;
+    g_clock_hz = 1e3 * (double)prop.clockRate;
     float* out;
     long long* cyc;
     CK(cudaMalloc(&out, sizeof(float) * sms * 8 * 256));
@@ -202,7 +289,25 @@ int main(int argc, char** argv) {
     run<DFMA>(sms, ctas, out, cyc, false);
     run<LDS128>(sms, ctas, out, cyc, false);
     run<FFMA2_FMUL>(sms, ctas, out, cyc, false);
-    run<FFMA2_MUFU_INDEP>(sms, ctas, out, cyc, true);
+    run<FFMA2_MUFU_INDEP>(sms, ctas, out, cyc, false);
+    run<FFMA2_3PAIRS>(sms, ctas, out, cyc, false);
+    run<FFMA2_UBCAST>(sms, ctas, out, cyc, false);
+    run<FFMA_3REGS>(sms, ctas, out, cyc, false);
+    run<SHARED_MIX>(sms, ctas, out, cyc, false);
+    int* map;  // 4096^2 int32 = 64 MB (config 3's map; fits the 126 MB L2) and 16384^2 = 1 GB (larger than L2)
+    for (int big = 0; big < 2; ++big) {
+        const unsigned n_pix = big ? (1u << 28) : (1u << 24);
+        CK(cudaMalloc(&map, sizeof(int) * (size_t)n_pix));
+        CK(cudaMemset(map, 0, sizeof(int) * (size_t)n_pix));
+        run_red<0>(big ? "red_random_1GB_map" : "red_random_64MB_map", sms, map, n_pix - 1, false);
+        run_red<3>(big ? "red_window32x32_1GB_map" : "red_window32x32_64MB_map", sms, map, n_pix - 1, false);
+        if (!big) {
+            run_red<1>("red_same_address_per_warp", sms, map, n_pix - 1, false);
+            run_red<2>("red_coalesced_neighbours", sms, map, n_pix - 1, false);
+        }
+        CK(cudaFree(map));
+    }
+    printf("  \"note\": \"rates are total work / event time at the maximum SM clock\"\n");
     printf("}\n");
     return 0;
 }

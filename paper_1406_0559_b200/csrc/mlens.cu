@@ -12,6 +12,7 @@
 #include <new>
 #include <vector>
 
+#include "mapstats_kernel.cuh"
 #include "shoot_kernel.cuh"
 
 namespace {
@@ -51,6 +52,8 @@ struct mlens {
     float4* lens_dev;                  // (x, y, m, 0)
     unsigned long long* counters_dev;  // in_map, outside, lost, total
     int* max_count_dev;
+    mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
+    mlk::MapStatsDev* mapstats_host;   // pinned mirror
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
     int* count_own;
@@ -99,6 +102,18 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         const long long cap = (long long)h->sm_count * 16;
         if (blocks > cap) blocks = cap;
         mlk::shoot_fp64_kernel<<<(unsigned)blocks, 256, 0, st>>>(P);
+        MLENS_CUDA(cudaGetLastError());
+        return MLENS_OK;
+    }
+
+    if (h->opt_kernel == 2) {  // ablation: plain-form FP32 (whole list resident in shared memory)
+        if (P.n_lens > 12000) return fail(MLENS_EINVAL, "kernel 2 (plain FP32 ablation) holds at most 12000 lenses");
+        const size_t smem = (size_t)(((P.n_lens + 3) & ~3) + 4) * 16;
+        const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
+        long long grid = (long long)h->sm_count * (smem > 100 * 1024 ? 1 : 2);
+        if (grid > n_tiles) grid = n_tiles;
+        MLENS_CUDA(cudaFuncSetAttribute(mlk::shoot_plain_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        mlk::shoot_plain_fp32_kernel<<<(unsigned)grid, 512, smem, st>>>(P);
         MLENS_CUDA(cudaGetLastError());
         return MLENS_OK;
     }
@@ -247,6 +262,8 @@ void mlens_destroy(mlens_t* h) {
     if (h->lens_dev) cudaFree(h->lens_dev);
     if (h->counters_dev) cudaFree(h->counters_dev);
     if (h->max_count_dev) cudaFree(h->max_count_dev);
+    if (h->mapstats_dev) cudaFree(h->mapstats_dev);
+    if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
     if (h->counters_host) cudaFreeHost(h->counters_host);
     if (h->count_own) cudaFree(h->count_own);
     if (h->mag_own) cudaFree(h->mag_own);
@@ -267,7 +284,7 @@ int mlens_get_geometry(const mlens_t* h, mlens_geometry* g) {
 int mlens_set_option(mlens_t* h, const char* key, long long value) {
     if (!h || !key) return fail(MLENS_EINVAL, "NULL argument");
     if (!strcmp(key, "kernel")) {
-        if (value < 0 || value > 1) return fail(MLENS_EINVAL, "kernel must be 0 or 1");
+        if (value < 0 || value > 2) return fail(MLENS_EINVAL, "kernel must be 0, 1 or 2");
         h->opt_kernel = (int)value;
     } else if (!strcmp(key, "binning")) {
         if (value < 0 || value > 3) return fail(MLENS_EINVAL, "binning must be 0..3");
@@ -310,6 +327,36 @@ int mlens_shoot_block(mlens_t* h, long long i0, long long j0, long long ni, long
 int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* cuda_stream) {
     if (!h || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
     return launch_magnification(h, count_dev, mag_dev, (cudaStream_t)cuda_stream);
+}
+
+int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, int n_bins, void* cuda_stream,
+              mlens_map_stats* stats) {
+    if (!h || !count_dev || !hist_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (n_bins < 2) return fail(MLENS_EINVAL, "n_bins must be >= 2");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!h->mapstats_dev) MLENS_CUDA(cudaMalloc(&h->mapstats_dev, sizeof(mlk::MapStatsDev)));
+    if (!h->mapstats_host) MLENS_CUDA(cudaMallocHost(&h->mapstats_host, sizeof(mlk::MapStatsDev)));
+    const long long n = (long long)h->npix * h->npix;
+    MLENS_CUDA(cudaMemsetAsync(h->mapstats_dev, 0, sizeof(mlk::MapStatsDev), st));
+    MLENS_CUDA(cudaMemsetAsync(hist_dev, 0, sizeof(unsigned long long) * (size_t)n_bins, st));
+    long long blocks = (n / 4 + mlk::kMpdThreads - 1) / mlk::kMpdThreads;
+    const long long cap = (long long)h->sm_count * 4;  // 4 x 256-thread CTAs per SM (32 KB shared memory each)
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, 0, st>>>(count_dev, n, hist_dev, n_bins, h->mapstats_dev);
+    MLENS_CUDA(cudaGetLastError());
+    if (stats) {
+        MLENS_CUDA(cudaMemcpyAsync(h->mapstats_host, h->mapstats_dev, sizeof(mlk::MapStatsDev), cudaMemcpyDeviceToHost, st));
+        MLENS_CUDA(cudaStreamSynchronize(st));
+        stats->n_pixels = n;
+        stats->sum_count = (long long)h->mapstats_host->sum_count;
+        stats->n_clamped = (long long)h->mapstats_host->n_clamped;
+        stats->min_count = 0x7fffffff - h->mapstats_host->inv_min_count;
+        stats->max_count = h->mapstats_host->max_count;
+        stats->mean_count = (double)stats->sum_count / (double)n;
+        stats->mean_mu = stats->mean_count / h->geo.n_avg;
+    }
+    return MLENS_OK;
 }
 
 int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, mlens_stats* stats) {

@@ -412,6 +412,92 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// ABLATION ONLY (mlens_set_option("kernel", 2)): the "obvious" FP32 kernel — Eq. (1) summed in plain FP32 in global
+// coordinates, same tiling, register blocking, packed arithmetic and MUFU reciprocal as the production kernel but no
+// difference form (5 packed FP32 instructions per ray pair instead of 6, no per-tile transform).  It exists to show
+// what the difference form buys: this kernel misses the north_star tolerances by 1-2 orders of magnitude
+// (tests/test_gpu_parity.py::test_plain_fp32_ablation_fails_the_tolerances).
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(512, 2) shoot_plain_fp32_kernel(const ShootParams P) {
+    constexpr int kR = 8, kThreads = 512, kTx = kTile / kR;
+    extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
+    float4* ls = reinterpret_cast<float4*>(smem_raw_bytes);  // whole lens list (x, y, m, 0), padded to a multiple of 4
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int tx = tid % kTx, ty = tid / kTx;
+    const int n_pad = (P.n_lens + 3) & ~3;
+    for (int t = tid; t < n_pad; t += kThreads) ls[t] = t < P.n_lens ? P.lens_raw[t] : make_float4(kFar, kFar, 0.f, 0.f);
+    __syncthreads();
+    const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
+    unsigned long long c_in = 0, c_out = 0, c_lost = 0;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
+        const long long jray = P.j0 + (long long)tJ * kTile + ty;
+        const long long iray0 = P.i0 + (long long)tI * kTile + tx * kR;
+        const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
+        const float x2f = (float)x2;
+        float2 xf[kR / 2], ax[kR / 2], ay[kR / 2];
+#pragma unroll
+        for (int j = 0; j < kR / 2; ++j) {
+            xf[j].x = (float)(((double)(iray0 + 2 * j) + 0.5 - P.half_n1) * P.d);
+            xf[j].y = (float)(((double)(iray0 + 2 * j + 1) + 0.5 - P.half_n1) * P.d);
+            ax[j] = ay[j] = make_float2(0.f, 0.f);
+        }
+#pragma unroll 4
+        for (int l = 0; l < n_pad; ++l) {
+            const float4 q = ls[l];
+            const float dy = x2f - q.y, dy2 = dy * dy;
+            const float2 NX = make_float2(-q.x, -q.x), DY2 = make_float2(dy2, dy2), M = make_float2(q.z, q.z);
+            const float2 DY = make_float2(dy, dy);
+#pragma unroll
+            for (int j = 0; j < kR / 2; ++j) {
+                const float2 dx = __fadd2_rn(xf[j], NX);
+                const float2 r2 = __ffma2_rn(dx, dx, DY2);
+                const float2 w = __fmul2_rn(M, make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y)));
+                ax[j] = __ffma2_rn(w, dx, ax[j]);
+                ay[j] = __ffma2_rn(w, DY, ay[j]);
+            }
+        }
+        int n_in = 0, n_out = 0, n_lost = 0;
+#pragma unroll
+        for (int k = 0; k < kR; ++k) {
+            const int j = k >> 1;
+            const long long iray = iray0 + k;
+            const bool ok = jray < P.j0 + P.nj && iray < P.i0 + P.ni;
+            const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
+            const double y1 = P.f1 * x1 - (double)((k & 1) ? ax[j].y : ax[j].x);
+            const double y2 = P.f2 * x2 - (double)((k & 1) ? ay[j].y : ay[j].x);
+            int pix;
+            if (!(isfinite(y1) && isfinite(y2))) {
+                pix = -2;
+            } else {
+                const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
+                pix = (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
+                          ? (int)floor(u2) * P.npix + (int)floor(u1) : -1;
+            }
+            if (ok) {
+                n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
+                if (P.ray_y || P.ray_pix) {
+                    const long long qidx = (jray - P.j0) * P.ni + (iray - P.i0);
+                    if (P.ray_y) { P.ray_y[2 * qidx] = y1; P.ray_y[2 * qidx + 1] = y2; }
+                    if (P.ray_pix) P.ray_pix[qidx] = pix;
+                }
+                if (P.count && pix >= 0) red_add(P.count + pix, 1);
+            }
+        }
+        n_in = __reduce_add_sync(0xffffffffu, n_in);
+        n_out = __reduce_add_sync(0xffffffffu, n_out);
+        n_lost = __reduce_add_sync(0xffffffffu, n_lost);
+        c_in += n_in; c_out += n_out; c_lost += n_lost;
+    }
+    if (lane == 0) {
+        if (c_in) atomicAdd(&P.counters[0], c_in);
+        if (c_out) atomicAdd(&P.counters[1], c_out);
+        if (c_lost) atomicAdd(&P.counters[2], c_lost);
+        if (c_in + c_out + c_lost) atomicAdd(&P.counters[3], c_in + c_out + c_lost);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // plumbing / debug kernel: Eq. (1) in plain FP64, one ray per thread, lenses read from global memory
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) shoot_fp64_kernel(const ShootParams P) {

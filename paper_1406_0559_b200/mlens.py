@@ -39,6 +39,15 @@ class Geometry(ctypes.Structure):
                 ("kappa_star", ctypes.c_double), ("n_avg", ctypes.c_double)]
 
 
+class MapStats(ctypes.Structure):
+    _fields_ = [("n_pixels", ctypes.c_longlong), ("sum_count", ctypes.c_longlong), ("n_clamped", ctypes.c_longlong),
+                ("min_count", ctypes.c_int), ("max_count", ctypes.c_int), ("mean_count", ctypes.c_double),
+                ("mean_mu", ctypes.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
 def lib() -> ctypes.CDLL:
     """Load libmlens.so and declare the prototypes of every symbol in include/mlens.h.  Raises if it is not built."""
     global _lib
@@ -53,6 +62,7 @@ def lib() -> ctypes.CDLL:
     L.mlens_shoot_block.argtypes = [vp, ll, ll, ll, ll, vp, vp, vp, vp]
     L.mlens_shoot_host.argtypes = [vp, vp, vp, ctypes.POINTER(Stats)]
     L.mlens_magnification.argtypes = [vp, vp, vp, vp]
+    L.mlens_mpd.argtypes = [vp, vp, vp, ci, vp, ctypes.POINTER(MapStats)]
     L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
     L.mlens_get_stats.argtypes = [vp, vp, ctypes.POINTER(Stats)]
     L.mlens_reset_stats.argtypes = [vp, vp]
@@ -61,7 +71,7 @@ def lib() -> ctypes.CDLL:
     L.mlens_last_error.restype = ctypes.c_char_p
     L.mlens_destroy.argtypes = [vp]
     L.mlens_destroy.restype = None
-    for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification",
+    for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
         getattr(L, name).restype = ci
     _lib = L
@@ -175,6 +185,20 @@ class Mlens:
         _check(lib().mlens_magnification(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(mag.data_ptr()),
                                          _stream_ptr(stream)))
         return mag
+
+    def mpd(self, count, n_bins, hist=None, stream=None, sync=True):
+        """mlens_mpd: histogram of the counts = the full MPD.  Returns (hist int64 [n_bins] on the
+        device — the library writes unsigned 64-bit bins, torch views them as int64 — and the map-stats dict or None)."""
+        import torch
+
+        if hist is None:
+            hist = torch.empty((int(n_bins),), dtype=torch.int64, device="cuda")
+        assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous() and hist.numel() == int(n_bins)
+        assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
+        ms = MapStats() if sync else None
+        _check(lib().mlens_mpd(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(hist.data_ptr()), int(n_bins),
+                               _stream_ptr(stream), ctypes.byref(ms) if sync else None))
+        return hist, (ms.as_dict() if sync else None)
 
     def stats(self, stream=None):
         st = Stats()

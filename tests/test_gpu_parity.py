@@ -284,3 +284,31 @@ def test_full_map_invariants(ml, oracle, cfg_id):
     print(f"cfg{cfg_id}: full map {st['elapsed_ms']:.1f} ms, <mu>/mu_th = {mean_mu / cfg.mu_th:.4f}, max count {st['max_count']}")
     if cfg_id in (3, 5):
         assert abs(mean_mu / cfg.mu_th - 1) < 0.15
+
+
+def test_plain_fp32_ablation_fails_the_tolerances(ml, oracle):
+    # "kernel" 2 sums Eq. 1 in plain FP32 in global coordinates (no difference form).  It is the evidence for
+    # same blocks, same oracle — the plain form misses the L1 budget that the production
+    # kernel meets with room to spare.  (The deflection tolerance (i) alone is loose enough for plain FP32.)
+    cfg = fields.CONFIGS[4]
+    xy, m = fields.lens_field(cfg)
+    res = {}
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        g = h.geometry
+        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 23, 4, 2, 0, size=192)
+        for kern in (1, 2):
+            h.set_option("kernel", kern)
+            l1 = in_map = 0
+            err = []
+            for b in blocks:
+                cnt = torch.zeros((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
+                out = h.shoot_block(*b, count=cnt, want_rays=True)
+                ref = oracle.shoot_block(*_args(cfg), xy, m, block=b, want_rays=True)
+                l1 += int(np.abs(cnt.cpu().numpy().astype(np.int64) - ref["count"]).sum())
+                in_map += ref["stats"]["rays_in_map"]
+                err.append(np.abs(out["y"].cpu().numpy() - ref["y"]).max() / cfg.pixel)
+            res[kern] = (l1 / max(1, in_map), max(err))
+    print(f"cfg4 ablation: difference form L1/in_map {res[1][0]:.2e} (max |dy| {res[1][1]:.2e} px); "
+          f"plain FP32 L1/in_map {res[2][0]:.2e} (max |dy| {res[2][1]:.2e} px)")
+    assert res[1][0] <= TOL_L1
+    assert res[2][0] > 10 * TOL_L1 and res[2][0] > 20 * max(res[1][0], 1e-6)
