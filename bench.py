@@ -352,6 +352,44 @@ def run_block(args):
                       "rays_in_map_frac": st["rays_in_map"] / max(1, st["rays_total"])}), flush=True)
 
 
+def run_mpd(args):
+    """--mpd: K launches of mlens_mpd (row f1: MPD histogram + map means) on the config's shot map; HBM roofline."""
+    import torch
+
+    from paper_1406_0559_b200 import mlens
+
+    torch.cuda.set_device(0)
+    cfg = fields.CONFIGS[args.config]
+    xy, m = fields.lens_field(cfg)
+    with mlens.Mlens.from_config(cfg, xy, m) as h:
+        count, _, st = h.shoot(want_mag=False)
+        n_bins = st["max_count"] + 2
+        hist = torch.empty((n_bins,), dtype=torch.int64, device="cuda")
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        for _ in range(args.warmup):
+            h.mpd(count, n_bins, hist=hist, sync=False)
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(args.steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            h.mpd(count, n_bins, hist=hist, sync=False)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        _, mst = h.mpd(count, n_bins, hist=hist)
+    med = statistics.median(ms)
+    nbytes = 4 * cfg.npix**2
+    peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(
+        os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+    gbs = nbytes / (med * 1e-3) / 1e9
+    print(json.dumps({"mode": "mpd", "config": args.config, "npix": cfg.npix, "n_bins": n_bins, "ms": ms, "ms_median": med,
+                      "algorithmic_bytes": nbytes, "achieved_gbs": gbs, "peak_gbs": peak, "frac": gbs / peak if peak else None,
+                      "note": "includes the memset of the bins and of the stats struct (stream-ordered, same events)",
+                      "map_stats": mst}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -362,9 +400,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--shard", action="store_true", help="N > 1: shoot ONE map in row bands + one all-reduce (strong scaling)")
     ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
+    ap.add_argument("--mpd", action="store_true", help="profile mode: time mlens_mpd on the config's shot map")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
     args = ap.parse_args()
-    if args.block:
+    if args.mpd:
+        run_mpd(args)
+    elif args.block:
         run_block(args)
     elif args.impl == "reference":
         run_reference(args)

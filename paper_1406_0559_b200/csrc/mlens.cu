@@ -54,6 +54,7 @@ struct mlens {
     int* max_count_dev;
     mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
     mlk::MapStatsDev* mapstats_host;   // pinned mirror
+    unsigned int* mpd_partial;         // sm_count x kMpdSmemBinsMax per-CTA histogram slices (lazily allocated)
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
     int* count_own;
@@ -264,6 +265,7 @@ void mlens_destroy(mlens_t* h) {
     if (h->max_count_dev) cudaFree(h->max_count_dev);
     if (h->mapstats_dev) cudaFree(h->mapstats_dev);
     if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
+    if (h->mpd_partial) cudaFree(h->mpd_partial);
     if (h->counters_host) cudaFreeHost(h->counters_host);
     if (h->count_own) cudaFree(h->count_own);
     if (h->mag_own) cudaFree(h->mag_own);
@@ -339,11 +341,20 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
     const long long n = (long long)h->npix * h->npix;
     MLENS_CUDA(cudaMemsetAsync(h->mapstats_dev, 0, sizeof(mlk::MapStatsDev), st));
     MLENS_CUDA(cudaMemsetAsync(hist_dev, 0, sizeof(unsigned long long) * (size_t)n_bins, st));
+    if (!h->mpd_partial)
+        MLENS_CUDA(cudaMalloc(&h->mpd_partial, sizeof(unsigned int) * (size_t)h->sm_count * mlk::kMpdSmemBinsMax));
+    // shared-memory bins: all of them when they fit (multiple of 1024 for the fill/flush loops), else the first 48 Ki
+    int smem_bins = (n_bins + 1023) & ~1023;
+    if (smem_bins > mlk::kMpdSmemBinsMax) smem_bins = mlk::kMpdSmemBinsMax;
     long long blocks = (n / 4 + mlk::kMpdThreads - 1) / mlk::kMpdThreads;
-    const long long cap = (long long)h->sm_count * 4;  // 4 x 256-thread CTAs per SM (32 KB shared memory each)
-    if (blocks > cap) blocks = cap;
+    if (blocks > h->sm_count) blocks = h->sm_count;  // one persistent 1024-thread CTA per SM
     if (blocks < 1) blocks = 1;
-    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, 0, st>>>(count_dev, n, hist_dev, n_bins, h->mapstats_dev);
+    const size_t smem = sizeof(unsigned int) * (size_t)smem_bins;
+    MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n, hist_dev, n_bins, smem_bins,
+                                                                       h->mpd_partial, h->mapstats_dev);
+    MLENS_CUDA(cudaGetLastError());
+    mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(h->mpd_partial, (int)blocks, smem_bins, hist_dev, n_bins);
     MLENS_CUDA(cudaGetLastError());
     if (stats) {
         MLENS_CUDA(cudaMemcpyAsync(h->mapstats_host, h->mapstats_dev, sizeof(mlk::MapStatsDev), cudaMemcpyDeviceToHost, st));

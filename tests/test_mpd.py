@@ -56,7 +56,7 @@ def test_p11_mpd_brute_force_invariants_and_clamping(oracle):
 # GPU parity
 # ---------------------------------------------------------------------------------------------------------------
 @pytest.mark.gpu
-@pytest.mark.parametrize("npix,n_bins,hi", [(64, 4096, 3000), (250, 100, 5000), (1023, 20000, 19000), (1, 2, 5), (2048, 9000, 40000)])
+@pytest.mark.parametrize("npix,n_bins,hi", [(64, 4096, 3000), (250, 100, 5000), (1023, 20000, 19000), (1, 2, 5), (2048, 9000, 40000), (512, 70000, 69000)])
 def test_mlens_mpd_matches_the_oracle_bit_for_bit(oracle, npix, n_bins, hi):
     import torch
 
