@@ -85,6 +85,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     P.f2 = 1.0 - h->geo.kappa_s + h->gamma;
     P.half_L = h->L / 2.0;
     P.p = h->geo.p;
+    P.inv_p = 1.0 / h->geo.p;
     P.npix = h->npix;
     P.lens_raw = h->lens_dev;
     P.n_lens = (int)h->n_lens;

@@ -18,8 +18,13 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#ifndef MLENS_HOT_UNROLL
+#define MLENS_HOT_UNROLL 12  // lenses per unrolled hot-loop iteration; 12 is the measured best of {1,2,4,6,8,12,16} (profiles/r1b_summary.md)
+#endif
+
 namespace mlk {
 
+constexpr int kHotUnroll = MLENS_HOT_UNROLL;
 constexpr int kTile = 64;           // tile is kTile x kTile rays
 constexpr int kMaxThreads = 512;    // threads per CTA = kTile*kTile/kR (kR rays per thread, consecutive along x1)
 constexpr int kNearMax = 32;        // capacity of the per-tile near-lens list
@@ -37,7 +42,7 @@ struct ShootParams {
     int tiles_x, tiles_y;
     // macro model and map
     double f1, f2;                  // 1-kappa_s-gamma, 1-kappa_s+gamma
-    double half_L, p;               // L/2, pixel size
+    double half_L, p, inv_p;        // L/2, pixel size and 1/p
     int npix;
     // lenses
     const float4* lens_raw;         // (x, y, m, 0) per lens, global memory
@@ -254,7 +259,7 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
 
             // (4) HOT LOOP: all lenses of the chunk x this thread's kR rays
             float4 qn = xf[0];
-#pragma unroll 4
+#pragma unroll kHotUnroll
             for (int l = 0; l < n_pad; ++l) {
                 const float4 q = qn;  // (zeta_x, zeta_y, c_r, c_i)
                 qn = xf[l + 1];       // broadcast LDS.128 one lens ahead (xf[n_pad] is readable: raw0 follows xf)
@@ -316,6 +321,20 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             __syncthreads();
         }
 
+        // Source position in PIXEL units, u = (y + L/2)/p.  Everything large is folded into one FP64 constant per tile,
+        //   U_c = (f * Z_c -+ A_c + L/2) / p,
+        // and a ray adds only its small in-tile part: u = U_c + (f*delta_true -+ delta*S)/p, where delta*S is formed in
+        // FP32 (its own rounding, ~1e-9 R_E, is below that of the S accumulators) and delta_true is the exact FP64
+        // in-tile offset.  One multiply by 1/p replaces the divide; against the oracle's (y + L/2)/p this moves u by
+        // a few ulp (1e-13 px), far inside the 1e-3 px exemption band of the parity tolerance.
+        const double U1c = (P.f1 * Zcx - Acr + P.half_L) * P.inv_p;
+        const double U2c = (P.f2 * Zcy + Aci + P.half_L) * P.inv_p;
+        const double dyt = ((double)ty - 31.5) * P.d;
+        const double row2 = P.f2 * dyt;
+        const bool special = n_near > 0 || near_overflow;  // tile-uniform: near-lens list or FP64 fallback in play
+        const bool want_rays = P.ray_y != nullptr || P.ray_pix != nullptr;
+        const double npix_d = (double)P.npix;
+
 #pragma unroll
         for (int k = 0; k < kR; ++k) {
             const int j = k >> 1;
@@ -324,46 +343,51 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             const float dxf = (k & 1) ? dxb[j].y : dxb[j].x;
             const long long iray = ti0 + tx * kR + k;
             const bool ok = row_ok && iray < P.i0 + P.ni;
-            const double dxd = (double)dxf, sr = (double)srf, si = (double)sif;
-            // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im)
-            double al1 = Acr - (dxd * sr - dyd * si);
-            double al2 = -(Aci - (dxd * si + dyd * sr));
-            for (int q = 0; q < n_near; ++q) {
-                const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyd;
-                const double f = sh.near_m[q] / (wx * wx + wy * wy);
-                al1 += f * wx;
-                al2 += f * wy;
-            }
-            const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
-            if (near_overflow) {
-                // more than kNearMax lenses within rho of this tile: the FP32 list then holds lenses it cannot sum
-                // accurately (or at all: r2 = 0), so the tile's rays take Eq. (1) in plain FP64 from global memory
-                al1 = al2 = 0.0;
-                for (int q = 0; q < P.n_lens; ++q) {
-                    const float4 l = __ldg(P.lens_raw + q);
-                    const double wx = x1 - (double)l.x, wy = x2 - (double)l.y;
-                    const double f = (double)l.z / (wx * wx + wy * wy);
+            // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im);  y1 = f1 x1 - alpha1,  y2 = f2 x2 - alpha2
+            const float ds_re = dxf * srf - dyf * sif;
+            const float ds_im = dxf * sif + dyf * srf;
+            const double dxt = ((double)(tx * kR + k) - 31.5) * P.d;
+            double u1 = fma(fma(P.f1, dxt, (double)ds_re), P.inv_p, U1c);
+            double u2 = fma(row2 - (double)ds_im, P.inv_p, U2c);
+            if (special) {
+                const double dxd = (double)dxf;
+                double al1 = Acr - (double)ds_re;
+                double al2 = -(Aci - (double)ds_im);
+                for (int q = 0; q < n_near; ++q) {
+                    const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyd;
+                    const double f = sh.near_m[q] / (wx * wx + wy * wy);
                     al1 += f * wx;
                     al2 += f * wy;
                 }
+                const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
+                if (near_overflow) {
+                    // more than kNearMax lenses within rho of this tile: the FP32 list then holds lenses it cannot sum
+                    // accurately (or at all: r2 = 0), so the tile's rays take Eq. (1) in plain FP64 from global memory
+                    al1 = al2 = 0.0;
+                    for (int q = 0; q < P.n_lens; ++q) {
+                        const float4 l = __ldg(P.lens_raw + q);
+                        const double wx = x1 - (double)l.x, wy = x2 - (double)l.y;
+                        const double f = (double)l.z / (wx * wx + wy * wy);
+                        al1 += f * wx;
+                        al2 += f * wy;
+                    }
+                }
+                u1 = (P.f1 * x1 - al1 + P.half_L) * P.inv_p;
+                u2 = (P.f2 * x2 - al2 + P.half_L) * P.inv_p;
             }
-            const double y1 = P.f1 * x1 - al1;
-            const double y2 = P.f2 * x2 - al2;
             int pix;
-            if (!(isfinite(y1) && isfinite(y2))) {
-                pix = -2;
+            if (!(fabs(u1) <= 1.7976931348623157e308 && fabs(u2) <= 1.7976931348623157e308)) {
+                pix = -2;  // non-finite source position (ray on a lens): lost
+            } else if (u1 >= 0.0 && u1 < npix_d && u2 >= 0.0 && u2 < npix_d) {
+                pix = (int)u2 * P.npix + (int)u1;  // u >= 0: truncation is floor
             } else {
-                const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
-                if (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
-                    pix = (int)floor(u2) * P.npix + (int)floor(u1);
-                else
-                    pix = -1;
+                pix = -1;
             }
             if (ok) {
                 n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
-                if (P.ray_y || P.ray_pix) {
+                if (want_rays) {
                     const long long qidx = (jray - P.j0) * P.ni + (iray - P.i0);
-                    if (P.ray_y) { P.ray_y[2 * qidx] = y1; P.ray_y[2 * qidx + 1] = y2; }
+                    if (P.ray_y) { P.ray_y[2 * qidx] = u1 * P.p - P.half_L; P.ray_y[2 * qidx + 1] = u2 * P.p - P.half_L; }
                     if (P.ray_pix) P.ray_pix[qidx] = pix;
                 }
             }
