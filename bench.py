@@ -390,6 +390,48 @@ def run_mpd(args):
                       "map_stats": mst}), flush=True)
 
 
+def run_convolve(args):
+    """--convolve: K launches of mlens_convolve (row f2, Eq. 6) on a map of the config's size (synthetic magnification
+    values: the convolution's cost does not depend on them); HBM roofline on the minimum traffic of the method."""
+    import torch
+
+    from paper_1406_0559_b200 import mlens
+
+    torch.cuda.set_device(0)
+    cfg = fields.CONFIGS[args.config]
+    n = cfg.npix
+    with mlens.Mlens.from_config(cfg, np.zeros((1, 2), np.float32), None) as h:
+        mag = torch.rand((n, n), dtype=torch.float32, device="cuda") * 4 + 0.5
+        ker = h.profile_kernel(1, max(1.0, n / 400.0))
+        out = torch.empty_like(mag)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        for _ in range(args.warmup):
+            h.convolve(mag, ker, out=out)
+        torch.cuda.synchronize()
+        ms = []
+        for _ in range(args.steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            h.convolve(mag, ker, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        flux = float(out.sum(dtype=torch.float64) / mag.sum(dtype=torch.float64))
+    med = statistics.median(ms)
+    nc = n * (n // 2 + 1)
+    # minimum HBM traffic of the method as built (each array touched once per stage): 2 R2C (read 4 B/pixel, write 8 B per
+    # complex) + product (read 2 x 8, write 8 per complex) + C2R (read 8 per complex, write 4 B/pixel)
+    nbytes = 2 * (4 * n * n + 8 * nc) + 24 * nc + (8 * nc + 4 * n * n)
+    peak_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    peak = json.load(open(peak_path)).get("hbm_gbs") if os.path.exists(peak_path) else None
+    gbs = nbytes / (med * 1e-3) / 1e9
+    print(json.dumps({"mode": "convolve", "config": args.config, "npix": n, "ms": ms, "ms_median": med,
+                      "min_stage_bytes": nbytes, "achieved_gbs": gbs, "peak_gbs": peak, "frac": gbs / peak if peak else None,
+                      "flux_ratio": flux, "paper_context": "~3 s per 10000^2 map with cuFFT on the paper's GPU (PAPER.md:152)"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -401,10 +443,13 @@ def main():
     ap.add_argument("--shard", action="store_true", help="N > 1: shoot ONE map in row bands + one all-reduce (strong scaling)")
     ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
     ap.add_argument("--mpd", action="store_true", help="profile mode: time mlens_mpd on the config's shot map")
+    ap.add_argument("--convolve", action="store_true", help="profile mode: time mlens_convolve on a map of the config's size")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
     args = ap.parse_args()
     if args.mpd:
         run_mpd(args)
+    elif args.convolve:
+        run_convolve(args)
     elif args.block:
         run_block(args)
     elif args.impl == "reference":

@@ -155,3 +155,30 @@ def mpd(count, n_bins, n_avg):
     mean = float(out[0]) / float(c.size)
     return hist, {"n_pixels": int(c.size), "sum_count": int(out[0]), "n_clamped": int(out[1]), "min_count": int(out[2]),
                   "max_count": int(out[3]), "mean_count": mean, "mean_mu": mean / float(n_avg)}
+
+
+def profile_kernel(shape, size, npix):
+    """Source-profile convolution kernel K (reading S19): float32 [npix, npix], sum 1, centre on (0,0)."""
+    K = np.empty((int(npix), int(npix)), dtype=np.float32)
+    lib().oracle_profile_kernel(ctypes.c_int(int(shape)), ctypes.c_double(float(size)), ctypes.c_int(int(npix)),
+                                _p(K, ctypes.c_float))
+    return K
+
+
+def convolve(M, K, points=None):
+    """Eq. 6 as its definition: circular convolution of float32 maps M and K in FP64.  points=None: the whole map
+    (float64 [npix, npix]); else an (n, 2) integer array of (y, x) output pixels -> float64 [n]."""
+    M = np.ascontiguousarray(M, dtype=np.float32)
+    K = np.ascontiguousarray(K, dtype=np.float32)
+    npix = M.shape[0]
+    assert M.shape == (npix, npix) == K.shape
+    if points is None:
+        out = np.empty((npix, npix), dtype=np.float64)
+        lib().oracle_convolve_at(_p(M, ctypes.c_float), _p(K, ctypes.c_float), ctypes.c_int(npix), None, ctypes.c_longlong(-1),
+                                 _p(out, ctypes.c_double))
+        return out
+    pts = np.ascontiguousarray(points, dtype=np.int64).reshape(-1, 2)
+    out = np.empty((pts.shape[0],), dtype=np.float64)
+    lib().oracle_convolve_at(_p(M, ctypes.c_float), _p(K, ctypes.c_float), ctypes.c_int(npix), _p(pts, ctypes.c_longlong),
+                             ctypes.c_longlong(pts.shape[0]), _p(out, ctypes.c_double))
+    return out

@@ -31,6 +31,7 @@
 // Build: g++ -O3 -march=native -fopenmp -shared -fPIC oracle/oracle.cpp -o oracle/liboracle.so   (no fast-math)
 
 #include <cmath>
+#include <vector>
 #include <cstdint>
 #include <cstring>
 #ifdef _OPENMP
@@ -214,6 +215,54 @@ void oracle_mpd(const int* count, long long n_pixels, unsigned long long* hist, 
         hist[b] += 1ull;
     }
     out[0] = sum; out[1] = clamped; out[2] = cmin; out[3] = cmax;
+}
+
+// Source-profile convolution kernel K ("the projected two-dimensional source profile is binned in
+// pixels of equal physical size to the map pixels, and then appended with empty (zero) pixels to match the pixel
+// dimensions of the map").  Reading S19: the profile is sampled at pixel centres, normalised to sum 1, its
+// centre sits on pixel (0,0) and negative offsets wrap to the far edge.  shape 0: uniform disc of radius `size`
+// pixels; shape 1: Gaussian of sigma `size` pixels, cut at 4 sigma.
+void oracle_profile_kernel(int shape, double size, int npix, float* K) {
+    std::vector<double> v((size_t)npix * npix, 0.0);
+    double sum = 0.0;
+    for (int iy = 0; iy < npix; ++iy) {
+        for (int ix = 0; ix < npix; ++ix) {
+            const int dx = ix <= npix / 2 ? ix : ix - npix, dy = iy <= npix / 2 ? iy : iy - npix;
+            const double r2 = (double)dx * dx + (double)dy * dy;
+            double p = 0.0;
+            if (shape == 0) p = (r2 <= size * size) ? 1.0 : 0.0;
+            else p = (r2 <= 16.0 * size * size) ? std::exp(-r2 / (2.0 * size * size)) : 0.0;
+            v[(size_t)iy * npix + ix] = p;
+            sum += p;
+        }
+    }
+    for (size_t q = 0; q < v.size(); ++q) K[q] = (float)(v[q] / sum);
+}
+
+// Eq. 6, C = M * K = F^-1[F(M) F(K)]: by the convolution theorem for the discrete transform this is the
+// CIRCULAR convolution, written out here as its definition, one requested output pixel at a time, in FP64:
+//   C[y][x] = sum_{y',x'} K[y'][x'] * M[(y - y') mod N][(x - x') mod N]
+// (only non-zero K entries contribute; the loop skips zeros).  pts = n_pts (y, x) pairs; n_pts < 0 => all N*N pixels in
+// row-major order.
+void oracle_convolve_at(const float* M, const float* K, int npix, const long long* pts, long long n_pts, double* out) {
+    std::vector<int> ky, kx;
+    std::vector<double> kv;
+    for (int y = 0; y < npix; ++y)
+        for (int x = 0; x < npix; ++x)
+            if (K[(size_t)y * npix + x] != 0.0f) { ky.push_back(y); kx.push_back(x); kv.push_back((double)K[(size_t)y * npix + x]); }
+    const long long n = n_pts < 0 ? (long long)npix * npix : n_pts;
+#pragma omp parallel for schedule(static)
+    for (long long q = 0; q < n; ++q) {
+        const int y = n_pts < 0 ? (int)(q / npix) : (int)pts[2 * q], x = n_pts < 0 ? (int)(q % npix) : (int)pts[2 * q + 1];
+        double acc = 0.0;
+        for (size_t t = 0; t < kv.size(); ++t) {
+            int yy = y - ky[t], xx = x - kx[t];
+            if (yy < 0) yy += npix;
+            if (xx < 0) xx += npix;
+            acc += kv[t] * (double)M[(size_t)yy * npix + xx];
+        }
+        out[q] = acc;
+    }
 }
 
 int oracle_max_threads(void) {

@@ -7,12 +7,12 @@ import sys
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "mlens.cu")
-DEPS = [SRC, os.path.join(_HERE, "csrc", "shoot_kernel.cuh"), os.path.join(_HERE, "csrc", "mapstats_kernel.cuh"),
+DEPS = [SRC, os.path.join(_HERE, "csrc", "shoot_kernel.cuh"), os.path.join(_HERE, "csrc", "mapstats_kernel.cuh"), os.path.join(_HERE, "csrc", "convolve_kernel.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "mlens.h")]
 OUT = os.path.join(_HERE, "lib", "libmlens.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared", "-Xcompiler",
-              "-fPIC", "-Xptxas", "-v"]
+              "-fPIC", "-Xptxas", "-v", "-lcufft", "-Xlinker", "-rpath=/usr/local/cuda/lib64"]
 
 
 MICRO_SRC = os.path.join(_HERE, "csrc", "alu_microbench.cu")

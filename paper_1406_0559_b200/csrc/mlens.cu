@@ -4,6 +4,7 @@
 #include "../../include/mlens.h"
 
 #include <cuda_runtime.h>
+#include <cufft.h>
 
 #include <cmath>
 #include <cstdarg>
@@ -12,6 +13,7 @@
 #include <new>
 #include <vector>
 
+#include "convolve_kernel.cuh"
 #include "mapstats_kernel.cuh"
 #include "shoot_kernel.cuh"
 
@@ -54,6 +56,11 @@ struct mlens {
     int* max_count_dev;
     mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
     mlk::MapStatsDev* mapstats_host;   // pinned mirror
+    // convolution (lazily created): cuFFT plans, spectra of the map and of the kernel, profile normalisation scratch
+    cufftHandle plan_r2c, plan_c2r;
+    int have_plans;
+    float2 *spec_map, *spec_ker;
+    double* prof_sum;
     unsigned int* mpd_partial;         // sm_count x kMpdSmemBinsMax per-CTA histogram slices (lazily allocated)
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
@@ -267,6 +274,10 @@ void mlens_destroy(mlens_t* h) {
     if (h->mapstats_dev) cudaFree(h->mapstats_dev);
     if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
     if (h->mpd_partial) cudaFree(h->mpd_partial);
+    if (h->have_plans) { cufftDestroy(h->plan_r2c); cufftDestroy(h->plan_c2r); }
+    if (h->spec_map) cudaFree(h->spec_map);
+    if (h->spec_ker) cudaFree(h->spec_ker);
+    if (h->prof_sum) cudaFree(h->prof_sum);
     if (h->counters_host) cudaFreeHost(h->counters_host);
     if (h->count_own) cudaFree(h->count_own);
     if (h->mag_own) cudaFree(h->mag_own);
@@ -368,6 +379,63 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
         stats->mean_count = (double)stats->sum_count / (double)n;
         stats->mean_mu = stats->mean_count / h->geo.n_avg;
     }
+    return MLENS_OK;
+}
+
+int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kernel_dev, void* cuda_stream) {
+    if (!h || !kernel_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (shape != mlk::PROFILE_UNIFORM_DISC && shape != mlk::PROFILE_GAUSSIAN) return fail(MLENS_EINVAL, "unknown profile shape %d", shape);
+    if (!std::isfinite(size_pixels) || !(size_pixels > 0)) return fail(MLENS_EINVAL, "profile size must be finite and > 0");
+    const double half = shape == mlk::PROFILE_GAUSSIAN ? std::ceil(4.0 * size_pixels) : std::ceil(size_pixels);
+    if (2.0 * half + 1.0 > (double)h->npix) return fail(MLENS_EINVAL, "profile support (%g pixels) does not fit the %d-pixel map", 2.0 * half + 1.0, h->npix);
+    const int R = (int)half;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!h->prof_sum) MLENS_CUDA(cudaMalloc(&h->prof_sum, sizeof(double)));
+    MLENS_CUDA(cudaMemsetAsync(h->prof_sum, 0, sizeof(double), st));
+    const long long ns = (2LL * R + 1) * (2LL * R + 1);
+    long long b1 = (ns + 255) / 256;
+    if (b1 > (long long)h->sm_count * 8) b1 = (long long)h->sm_count * 8;
+    mlk::profile_sum_kernel<<<(unsigned)b1, 256, 0, st>>>(shape, size_pixels, R, h->prof_sum);
+    MLENS_CUDA(cudaGetLastError());
+    const long long n = (long long)h->npix * h->npix;
+    long long b2 = (n + 255) / 256;
+    if (b2 > (long long)h->sm_count * 8) b2 = (long long)h->sm_count * 8;
+    mlk::profile_fill_kernel<<<(unsigned)b2, 256, 0, st>>>(shape, size_pixels, R, h->npix, h->prof_sum, kernel_dev);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+#define MLENS_CUFFT(call)                                                                   \
+    do {                                                                                    \
+        cufftResult r_ = (call);                                                            \
+        if (r_ != CUFFT_SUCCESS)                                                            \
+            return fail(r_ == CUFFT_ALLOC_FAILED ? MLENS_ENOMEM : MLENS_ECUDA, "%s: cuFFT error %d", #call, (int)r_); \
+    } while (0)
+
+int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, float* out_dev, void* cuda_stream) {
+    if (!h || !map_dev || !kernel_dev || !out_dev) return fail(MLENS_EINVAL, "NULL argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = h->npix;
+    const long long nc = (long long)N * (N / 2 + 1);  // complex elements of an R2C spectrum
+    if (!h->have_plans) {
+        MLENS_CUFFT(cufftPlan2d(&h->plan_r2c, N, N, CUFFT_R2C));
+        cufftResult r = cufftPlan2d(&h->plan_c2r, N, N, CUFFT_C2R);
+        if (r != CUFFT_SUCCESS) { cufftDestroy(h->plan_r2c); return fail(MLENS_ECUDA, "cufftPlan2d(C2R): cuFFT error %d", (int)r); }
+        h->have_plans = 1;
+    }
+    if (!h->spec_map) MLENS_CUDA(cudaMalloc(&h->spec_map, sizeof(float2) * (size_t)nc));
+    if (!h->spec_ker) MLENS_CUDA(cudaMalloc(&h->spec_ker, sizeof(float2) * (size_t)nc));
+    MLENS_CUFFT(cufftSetStream(h->plan_r2c, st));
+    MLENS_CUFFT(cufftSetStream(h->plan_c2r, st));
+    // out-of-place R2C leaves its real input untouched; cuFFT takes non-const pointers
+    MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(map_dev), reinterpret_cast<cufftComplex*>(h->spec_map)));
+    MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_ker)));
+    long long blocks = (nc / 2 + 255) / 256;
+    if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    mlk::spectral_product_kernel<<<(unsigned)blocks, 256, 0, st>>>(h->spec_map, h->spec_ker, nc, 1.0f / ((float)N * (float)N));
+    MLENS_CUDA(cudaGetLastError());
+    MLENS_CUFFT(cufftExecC2R(h->plan_c2r, reinterpret_cast<cufftComplex*>(h->spec_map), out_dev));
     return MLENS_OK;
 }
 

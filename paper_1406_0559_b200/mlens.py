@@ -63,6 +63,8 @@ def lib() -> ctypes.CDLL:
     L.mlens_shoot_host.argtypes = [vp, vp, vp, ctypes.POINTER(Stats)]
     L.mlens_magnification.argtypes = [vp, vp, vp, vp]
     L.mlens_mpd.argtypes = [vp, vp, vp, ci, vp, ctypes.POINTER(MapStats)]
+    L.mlens_profile_kernel.argtypes = [vp, ci, dbl, vp, vp]
+    L.mlens_convolve.argtypes = [vp, vp, vp, vp, vp]
     L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
     L.mlens_get_stats.argtypes = [vp, vp, ctypes.POINTER(Stats)]
     L.mlens_reset_stats.argtypes = [vp, vp]
@@ -72,6 +74,7 @@ def lib() -> ctypes.CDLL:
     L.mlens_destroy.argtypes = [vp]
     L.mlens_destroy.restype = None
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
+                 "mlens_profile_kernel", "mlens_convolve",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
         getattr(L, name).restype = ci
     _lib = L
@@ -199,6 +202,30 @@ class Mlens:
         _check(lib().mlens_mpd(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(hist.data_ptr()), int(n_bins),
                                _stream_ptr(stream), ctypes.byref(ms) if sync else None))
         return hist, (ms.as_dict() if sync else None)
+
+    def profile_kernel(self, shape: int, size_pixels: float, kernel=None, stream=None):
+        """mlens_profile_kernel: convolution kernel of a source profile (0 uniform disc, 1 Gaussian), float32 [npix,npix]."""
+        import torch
+
+        if kernel is None:
+            kernel = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
+        assert kernel.is_cuda and kernel.dtype == torch.float32 and kernel.is_contiguous() and kernel.numel() == self.npix**2
+        _check(lib().mlens_profile_kernel(self._h, int(shape), float(size_pixels), ctypes.c_void_p(kernel.data_ptr()),
+                                          _stream_ptr(stream)))
+        return kernel
+
+    def convolve(self, mag, kernel, out=None, stream=None):
+        """mlens_convolve: out = F^-1[F(mag) F(kernel)] (Eq. 6), the circular convolution; float32 [npix,npix]."""
+        import torch
+
+        if out is None:
+            out = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
+        for t in (mag, kernel, out):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.npix**2
+        assert out.data_ptr() not in (mag.data_ptr(), kernel.data_ptr())
+        _check(lib().mlens_convolve(self._h, ctypes.c_void_p(mag.data_ptr()), ctypes.c_void_p(kernel.data_ptr()),
+                                    ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+        return out
 
     def stats(self, stream=None):
         st = Stats()
