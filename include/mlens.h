@@ -120,6 +120,24 @@ int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* 
 int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, int n_bins, void* cuda_stream,
               mlens_map_stats* stats);
 
+/* Indexed maps: "The index file will hold all the distinct ray-count values,
+ * each matched to an index running from zero to the maximum number of distinct ray-counts in the map.  The indexed map
+ * will have its pixel ray-count values replaced by the appropriate index" — stored in 16 bits, halving the map.
+ *   count_dev    DEVICE npix*npix int32 (a finished count map, counts >= 0)
+ *   values_dev   DEVICE max_values int32, caller-owned: the index file, distinct counts in ASCENDING order
+ *   indexed_dev  DEVICE npix*npix unsigned 16-bit, caller-owned: index of every pixel's count
+ *   n_distinct   HOST out: number of distinct values (bits needed = ceil(log2(n_distinct)), PAPER.md Table B.6)
+ * Synchronises `cuda_stream` (the distinct count comes back to the host).  Integer-exact and lossless:
+ * mlens_unindex_map(indexed, values) reproduces count_dev bit for bit.  MLENS_ERANGE if the map has more than 65536
+ * distinct values (the paper's maximum over ~70 000 maps is 58 042, Table B.5) or more than max_values; *n_distinct is
+ * set in both cases. */
+int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_values, unsigned short* indexed_dev,
+                    void* cuda_stream, int* n_distinct);
+
+/* Decode: count_dev[q] = values_dev[indexed_dev[q]] (-1 for an index >= n_values).  Asynchronous. */
+int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* values_dev, int n_values, int* count_dev,
+                      void* cuda_stream);
+
 /* Finite-source convolution (Eq. 6): C = M * K = F^-1[F(M) F(K)].
  *
  * mlens_profile_kernel writes the convolution kernel K of a source profile: the profile is sampled at pixel centres

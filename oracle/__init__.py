@@ -182,3 +182,14 @@ def convolve(M, K, points=None):
     lib().oracle_convolve_at(_p(M, ctypes.c_float), _p(K, ctypes.c_float), ctypes.c_int(npix), _p(pts, ctypes.c_longlong),
                              ctypes.c_longlong(pts.shape[0]), _p(out, ctypes.c_double))
     return out
+
+
+def index_map(count):
+    """Indexed map + index file.  Returns (values int32 [n_distinct] ascending, indexed int32 map)."""
+    c = np.ascontiguousarray(count, dtype=np.int32)
+    values = np.empty((c.size,), dtype=np.int32)
+    indexed = np.empty(c.shape, dtype=np.int32)
+    f = lib().oracle_index_map
+    f.restype = ctypes.c_longlong
+    n = f(_p(c, ctypes.c_int), ctypes.c_longlong(c.size), _p(values, ctypes.c_int), _p(indexed, ctypes.c_int))
+    return values[:n].copy(), indexed

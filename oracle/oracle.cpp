@@ -30,6 +30,7 @@
 //
 // Build: g++ -O3 -march=native -fopenmp -shared -fPIC oracle/oracle.cpp -o oracle/liboracle.so   (no fast-math)
 
+#include <algorithm>
 #include <cmath>
 #include <vector>
 #include <cstdint>
@@ -263,6 +264,19 @@ void oracle_convolve_at(const float* M, const float* K, int npix, const long lon
         }
         out[q] = acc;
     }
+}
+
+// Indexed map: index file = the distinct ray-count values (ascending), indexed map = every pixel's
+// count replaced by its position in the index file.  Plain sort + unique + binary search.  Returns the number of
+// distinct values (values must hold n_pixels entries at most; indexed holds 32-bit indices here).
+long long oracle_index_map(const int* count, long long n_pixels, int* values, int* indexed) {
+    std::vector<int> v(count, count + n_pixels);
+    std::sort(v.begin(), v.end());
+    v.erase(std::unique(v.begin(), v.end()), v.end());
+    for (size_t k = 0; k < v.size(); ++k) values[k] = v[k];
+    for (long long q = 0; q < n_pixels; ++q)
+        indexed[q] = (int)(std::lower_bound(v.begin(), v.end(), count[q]) - v.begin());
+    return (long long)v.size();
 }
 
 int oracle_max_threads(void) {

@@ -142,3 +142,89 @@ __global__ void __launch_bounds__(256) mpd_reduce_kernel(const unsigned int* __r
 }
 
 }  // namespace mlk
+
+// ---------------------------------------------------------------------------------------------------------------
+// Indexed maps: "convert a map with ray-counts to an indexed map and an index
+// file.  The index file will hold all the distinct ray-count values, each matched to an index running from zero ...
+// The indexed map will have its pixel ray-count values replaced by the appropriate index", stored in 16 bits.
+// The distinct values are the non-empty bins of the MPD histogram, so the index file is a stream compaction of it.
+// ---------------------------------------------------------------------------------------------------------------
+namespace mlk {
+
+// One CTA: exclusive scan of (hist[b] != 0) over all bins -> lut[b] = index of count value b (or -1), values[index] = b
+// in ascending order, *n_distinct = number of non-empty bins.  n_bins <= ~1e6, so a single 1024-thread CTA walking the
+// bins in 1024-wide strips with a running offset is enough (a few tens of microseconds).
+__global__ void __launch_bounds__(1024, 1) index_build_kernel(const unsigned long long* __restrict__ hist, int n_bins,
+                                                              int* __restrict__ lut, int* __restrict__ values,
+                                                              int max_values, int* __restrict__ n_distinct) {
+    __shared__ int warp_sums[32];
+    __shared__ int base;
+    if (threadIdx.x == 0) base = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int b0 = 0; b0 < n_bins; b0 += 1024) {
+        const int b = b0 + threadIdx.x;
+        const int flag = (b < n_bins && hist[b] != 0ull) ? 1 : 0;
+        int incl = flag;  // inclusive warp scan
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, off);
+            if (lane >= off) incl += t;
+        }
+        if (lane == 31) warp_sums[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            int w = warp_sums[lane], wi = w;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, wi, off);
+                if (lane >= off) wi += t;
+            }
+            warp_sums[lane] = wi - w;  // exclusive offsets of the warps
+        }
+        __syncthreads();
+        const int idx = base + warp_sums[warp] + incl - flag;
+        if (b < n_bins) {
+            lut[b] = flag ? idx : -1;
+            if (flag && idx < max_values) values[idx] = b;
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) base = idx + flag;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *n_distinct = base;
+}
+
+// indexed[q] = lut[count[q]] as 16-bit; 4 pixels per thread per iteration (int4 in, 8 bytes out): 6 B/pixel of HBM
+// traffic, the LUT (4 B x n_bins) is served from L1/L2.
+__global__ void __launch_bounds__(256) index_apply_kernel(const int* __restrict__ count, long long n, const int* __restrict__ lut,
+                                                          unsigned short* __restrict__ indexed) {
+    const long long n4 = n >> 2, stride = (long long)gridDim.x * 256;
+    for (long long q = (long long)blockIdx.x * 256 + threadIdx.x; q < n4; q += stride) {
+        const int4 c = __ldg(reinterpret_cast<const int4*>(count) + q);
+        ushort4 o;
+        // counts are >= 0 by construction; max(c, 0) keeps a corrupt negative from reading outside the table
+        o.x = (unsigned short)__ldg(lut + max(c.x, 0)); o.y = (unsigned short)__ldg(lut + max(c.y, 0));
+        o.z = (unsigned short)__ldg(lut + max(c.z, 0)); o.w = (unsigned short)__ldg(lut + max(c.w, 0));
+        reinterpret_cast<ushort4*>(indexed)[q] = o;
+    }
+    for (long long q = (n4 << 2) + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride)
+        indexed[q] = (unsigned short)__ldg(lut + max(count[q], 0));
+}
+
+// count[q] = values[indexed[q]] (the decode direction)
+__global__ void __launch_bounds__(256) index_decode_kernel(const unsigned short* __restrict__ indexed, long long n,
+                                                           const int* __restrict__ values, int n_values, int* __restrict__ count) {
+    const long long n4 = n >> 2, stride = (long long)gridDim.x * 256;
+    for (long long q = (long long)blockIdx.x * 256 + threadIdx.x; q < n4; q += stride) {
+        const ushort4 i = __ldg(reinterpret_cast<const ushort4*>(indexed) + q);
+        int4 c;
+        c.x = i.x < n_values ? __ldg(values + i.x) : -1; c.y = i.y < n_values ? __ldg(values + i.y) : -1;
+        c.z = i.z < n_values ? __ldg(values + i.z) : -1; c.w = i.w < n_values ? __ldg(values + i.w) : -1;
+        reinterpret_cast<int4*>(count)[q] = c;
+    }
+    for (long long q = (n4 << 2) + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride)
+        count[q] = indexed[q] < n_values ? __ldg(values + indexed[q]) : -1;
+}
+
+}  // namespace mlk

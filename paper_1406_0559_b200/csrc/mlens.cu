@@ -61,6 +61,10 @@ struct mlens {
     int have_plans;
     float2 *spec_map, *spec_ker;
     double* prof_sum;
+    unsigned long long* idx_hist;      // scratch of mlens_index_map: histogram, LUT, distinct counter
+    int* idx_lut;
+    long long idx_bins_cap;
+    int* idx_n_dev;
     unsigned int* mpd_partial;         // sm_count x kMpdSmemBinsMax per-CTA histogram slices (lazily allocated)
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
@@ -274,6 +278,9 @@ void mlens_destroy(mlens_t* h) {
     if (h->mapstats_dev) cudaFree(h->mapstats_dev);
     if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
     if (h->mpd_partial) cudaFree(h->mpd_partial);
+    if (h->idx_hist) cudaFree(h->idx_hist);
+    if (h->idx_lut) cudaFree(h->idx_lut);
+    if (h->idx_n_dev) cudaFree(h->idx_n_dev);
     if (h->have_plans) { cufftDestroy(h->plan_r2c); cufftDestroy(h->plan_c2r); }
     if (h->spec_map) cudaFree(h->spec_map);
     if (h->spec_ker) cudaFree(h->spec_ker);
@@ -379,6 +386,62 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
         stats->mean_count = (double)stats->sum_count / (double)n;
         stats->mean_mu = stats->mean_count / h->geo.n_avg;
     }
+    return MLENS_OK;
+}
+
+int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_values, unsigned short* indexed_dev,
+                    void* cuda_stream, int* n_distinct) {
+    if (!h || !count_dev || !values_dev || !indexed_dev || !n_distinct) return fail(MLENS_EINVAL, "NULL argument");
+    if (max_values < 1) return fail(MLENS_EINVAL, "max_values must be >= 1");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long n = (long long)h->npix * h->npix;
+    // (1) largest count -> number of histogram bins
+    if (int rc = launch_magnification(h, count_dev, nullptr, st)) return rc;
+    MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 4, h->max_count_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    MLENS_CUDA(cudaStreamSynchronize(st));
+    int max_count;
+    memcpy(&max_count, h->counters_host + 4, sizeof(int));
+    const long long n_bins = (long long)max_count + 2;
+    if (n_bins > h->idx_bins_cap) {
+        if (h->idx_hist) cudaFree(h->idx_hist);
+        if (h->idx_lut) cudaFree(h->idx_lut);
+        h->idx_hist = nullptr; h->idx_lut = nullptr; h->idx_bins_cap = 0;
+        MLENS_CUDA(cudaMalloc(&h->idx_hist, sizeof(unsigned long long) * (size_t)n_bins));
+        MLENS_CUDA(cudaMalloc(&h->idx_lut, sizeof(int) * (size_t)n_bins));
+        h->idx_bins_cap = n_bins;
+    }
+    if (!h->idx_n_dev) MLENS_CUDA(cudaMalloc(&h->idx_n_dev, sizeof(int)));
+    // (2) the MPD histogram: its non-empty bins are the distinct ray-count values
+    if (int rc = mlens_mpd(h, count_dev, h->idx_hist, (int)n_bins, cuda_stream, nullptr)) return rc;
+    // (3) compaction -> index file (values, ascending) and the count -> index table
+    mlk::index_build_kernel<<<1, 1024, 0, st>>>(h->idx_hist, (int)n_bins, h->idx_lut, values_dev, max_values, h->idx_n_dev);
+    MLENS_CUDA(cudaGetLastError());
+    MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 5, h->idx_n_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+    MLENS_CUDA(cudaStreamSynchronize(st));
+    int nd;
+    memcpy(&nd, h->counters_host + 5, sizeof(int));
+    *n_distinct = nd;
+    if (nd > 65536) return fail(MLENS_ERANGE, "%d distinct ray-count values do not fit a 16-bit index", nd);
+    if (nd > max_values) return fail(MLENS_ERANGE, "%d distinct ray-count values, values_dev holds %d", nd, max_values);
+    // (4) the indexed map
+    long long blocks = (n / 4 + 255) / 256;
+    if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    mlk::index_apply_kernel<<<(unsigned)blocks, 256, 0, st>>>(count_dev, n, h->idx_lut, indexed_dev);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* values_dev, int n_values, int* count_dev,
+                      void* cuda_stream) {
+    if (!h || !indexed_dev || !values_dev || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (n_values < 1 || n_values > 65536) return fail(MLENS_EINVAL, "n_values must be 1..65536");
+    const long long n = (long long)h->npix * h->npix;
+    long long blocks = (n / 4 + 255) / 256;
+    if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
+    if (blocks < 1) blocks = 1;
+    mlk::index_decode_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(indexed_dev, n, values_dev, n_values, count_dev);
+    MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }
 

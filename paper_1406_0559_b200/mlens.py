@@ -63,6 +63,8 @@ def lib() -> ctypes.CDLL:
     L.mlens_shoot_host.argtypes = [vp, vp, vp, ctypes.POINTER(Stats)]
     L.mlens_magnification.argtypes = [vp, vp, vp, vp]
     L.mlens_mpd.argtypes = [vp, vp, vp, ci, vp, ctypes.POINTER(MapStats)]
+    L.mlens_index_map.argtypes = [vp, vp, vp, ci, vp, vp, ctypes.POINTER(ci)]
+    L.mlens_unindex_map.argtypes = [vp, vp, vp, ci, vp, vp]
     L.mlens_profile_kernel.argtypes = [vp, ci, dbl, vp, vp]
     L.mlens_convolve.argtypes = [vp, vp, vp, vp, vp]
     L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
@@ -74,7 +76,7 @@ def lib() -> ctypes.CDLL:
     L.mlens_destroy.argtypes = [vp]
     L.mlens_destroy.restype = None
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
-                 "mlens_profile_kernel", "mlens_convolve",
+                 "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
         getattr(L, name).restype = ci
     _lib = L
@@ -202,6 +204,30 @@ class Mlens:
         _check(lib().mlens_mpd(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(hist.data_ptr()), int(n_bins),
                                _stream_ptr(stream), ctypes.byref(ms) if sync else None))
         return hist, (ms.as_dict() if sync else None)
+
+    def index_map(self, count, max_values=65536, stream=None):
+        """mlens_index_map: (values int32 [n_distinct] ascending, indexed uint16 [npix,npix]) — PAPER.md:700-706."""
+        import torch
+
+        assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
+        values = torch.empty((int(max_values),), dtype=torch.int32, device="cuda")
+        indexed = torch.empty((self.npix, self.npix), dtype=torch.uint16, device="cuda")
+        nd = ctypes.c_int(0)
+        _check(lib().mlens_index_map(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(values.data_ptr()),
+                                     int(max_values), ctypes.c_void_p(indexed.data_ptr()), _stream_ptr(stream), ctypes.byref(nd)))
+        return values[: nd.value], indexed
+
+    def unindex_map(self, indexed, values, count=None, stream=None):
+        """mlens_unindex_map: count[q] = values[indexed[q]]."""
+        import torch
+
+        if count is None:
+            count = torch.empty((self.npix, self.npix), dtype=torch.int32, device="cuda")
+        assert indexed.is_cuda and indexed.dtype == torch.uint16 and indexed.is_contiguous() and indexed.numel() == self.npix**2
+        assert values.is_cuda and values.dtype == torch.int32 and values.is_contiguous()
+        _check(lib().mlens_unindex_map(self._h, ctypes.c_void_p(indexed.data_ptr()), ctypes.c_void_p(values.data_ptr()),
+                                       int(values.numel()), ctypes.c_void_p(count.data_ptr()), _stream_ptr(stream)))
+        return count
 
     def profile_kernel(self, shape: int, size_pixels: float, kernel=None, stream=None):
         """mlens_profile_kernel: convolution kernel of a source profile (0 uniform disc, 1 Gaussian), float32 [npix,npix]."""

@@ -98,3 +98,59 @@ def test_mpd_of_a_shot_map_ties_to_the_ray_counters(oracle):
         assert int(hist.sum().item()) == cfg.npix**2
         ref_hist, _ = oracle.mpd(count.cpu().numpy(), st["max_count"] + 2, h.geometry.n_avg)
         assert np.array_equal(hist.cpu().numpy().astype(np.uint64), ref_hist)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# indexed maps
+# ---------------------------------------------------------------------------------------------------------------
+def test_p13_index_map_oracle_brute_force_and_roundtrip(oracle):
+    count = np.array([[7, 3, 7, 100], [3, 3, 0, 100], [5, 7, 65000, 0]], np.int32)
+    values, indexed = oracle.index_map(count)
+    assert values.tolist() == [0, 3, 5, 7, 100, 65000]  # the index file: distinct values, ascending (by hand)
+    assert indexed.tolist() == [[3, 1, 3, 4], [1, 1, 0, 4], [2, 3, 5, 0]]
+    rng = np.random.default_rng(3)
+    count = (rng.integers(0, 300, size=(40, 33)) * rng.integers(1, 4, size=(40, 33))).astype(np.int32)
+    values, indexed = oracle.index_map(count)
+    lookup = {v: k for k, v in enumerate(sorted(set(count.reshape(-1).tolist())))}  # pure-Python restatement
+    assert values.tolist() == sorted(lookup) and indexed.tolist() == [[lookup[v] for v in row] for row in count.tolist()]
+    assert np.array_equal(values[indexed], count)  # lossless ("without any loss of information")
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("npix,hi", [(64, 3000), (1023, 19000), (3, 5), (2048, 900000)])
+def test_index_map_matches_the_oracle_and_roundtrips(oracle, npix, hi):
+    import torch
+
+    from paper_1406_0559_b200 import mlens
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    u = fields.uniform01(21 + npix, 0, npix * npix)
+    count = (200 + 30 * np.sin(np.arange(npix * npix) * 1e-3) + (u > 0.98) * u * hi).astype(np.int32).reshape(npix, npix)
+    count[0, 0] = 0
+    cfg = fields.MapConfig("idx", npix, 4.0, 0.3, 0.1, 0.0, 5, "unit", 3)
+    with mlens.Mlens.from_config(cfg, np.zeros((1, 2), np.float32), None) as h:
+        c_dev = torch.from_numpy(count).cuda()
+        values, indexed = h.index_map(c_dev)
+        ref_values, ref_indexed = oracle.index_map(count)
+        assert np.array_equal(values.cpu().numpy(), ref_values)
+        assert np.array_equal(indexed.cpu().numpy().astype(np.int32), ref_indexed)
+        back = h.unindex_map(indexed, values.contiguous())
+        assert torch.equal(back, c_dev)
+
+
+@pytest.mark.gpu
+def test_index_map_reports_too_many_distinct_values():
+    import torch
+
+    from paper_1406_0559_b200 import mlens
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    npix = 300  # 90 000 pixels, all different
+    cfg = fields.MapConfig("idx", npix, 4.0, 0.3, 0.1, 0.0, 5, "unit", 3)
+    with mlens.Mlens.from_config(cfg, np.zeros((1, 2), np.float32), None) as h:
+        c_dev = torch.arange(npix * npix, dtype=torch.int32, device="cuda").reshape(npix, npix).contiguous()
+        with pytest.raises(mlens.MlensError) as e:
+            h.index_map(c_dev)
+        assert e.value.code == mlens.ERANGE
