@@ -148,12 +148,14 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     void (*kern)(const mlk::ShootParams) = nullptr;
     const int code = h->opt_rays * 100 + h->opt_shared;
     switch (code) {
-#define MLENS_VARIANT(R, SH) case R * 100 + SH: kern = mlk::shoot_fp32_kernel<R, SH>; break;
+#define MLENS_VARIANT(R, SH) case R * 100 + SH: kern = mlk::shoot_fp32_kernel<R, SH, -1>; break;
         MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
         MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2)
 #undef MLENS_VARIANT
         default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d shared_rcp=%d", h->opt_rays, h->opt_shared);
     }
+    // the production configuration has its binning route compiled in (shorter epilogue)
+    if (code == 800 && h->opt_binning == mlk::BIN_RUNS) kern = mlk::shoot_fp32_kernel<8, 0, mlk::BIN_RUNS>;
     const int threads = mlk::kTile * mlk::kTile / h->opt_rays;
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)grid, threads, smem, st>>>(P);

@@ -19,7 +19,7 @@
 #include <stdint.h>
 
 #ifndef MLENS_HOT_UNROLL
-#define MLENS_HOT_UNROLL 12  // lenses per unrolled hot-loop iteration; 12 is the measured best of {1,2,4,6,8,12,16} (profiles/r1b_summary.md)
+#define MLENS_HOT_UNROLL 24  // lenses per unrolled hot-loop iteration; measured best of {1,2,4,6,8,12,16,24} (profiles/r1c_summary.md)
 #endif
 
 namespace mlk {
@@ -126,11 +126,11 @@ struct __align__(16) TileShared {
 };
 
 // a finished run (pix, n) of one thread goes to the map by the selected route; called convergently by the whole warp
-__device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, int pix, int n, bool active) {
-    if (P.bin_mode == BIN_WARP) {
+__device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, int bin_mode, int pix, int n, bool active) {
+    if (bin_mode == BIN_WARP) {
         warp_aggregated_add(P.count, pix, n, active);
     } else if (active) {
-        if (P.bin_mode == BIN_RUNS) {
+        if (bin_mode == BIN_RUNS) {
             red_add(P.count + pix, n);
         } else {  // BIN_WINDOW: CTA-private shared-memory window, global RED for strays
             const int wx = pix % P.npix - sh.win_ix0, wy = pix / P.npix - sh.win_iy0;
@@ -148,8 +148,10 @@ __device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, 
 // Kept as an ablation switch only: measured on B200 it LOSES (150.7 -> 159.2 -> 175.8 ms for 0/1/2 shared groups,
 // profiles/r1_summary.md).  Packed FP32 instructions with three distinct register-pair operands are bound by
 // register-file read bandwidth (3.0 clk, not 2.0), so the three extra FMUL2 cost more than the two MUFU they save.
-template <int kR, int kShared>
+// kBin >= 0 fixes the binning route at compile time (the production instantiation: BIN_RUNS); kBin < 0 reads P.bin_mode.
+template <int kR, int kShared, int kBin>
 __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const ShootParams P) {
+    const int bin_mode = kBin >= 0 ? kBin : P.bin_mode;
     constexpr int kThreads = kTile * kTile / kR;
     constexpr int kTx = kTile / kR;  // threads along x1
     extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
@@ -309,7 +311,7 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
         int n_in = 0, n_out = 0, n_lost = 0;
         int run_pix = -1, run_n = 0;
 
-        if (P.bin_mode == BIN_WINDOW) {
+        if (bin_mode == BIN_WINDOW) {
             // window origin: pixel of the tile centre under the macro-model plus the tile-centre deflection
             if (tid == 0) {
                 const double yc1 = P.f1 * Zcx - Acr, yc2 = P.f2 * Zcy + Aci;
@@ -393,17 +395,17 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             }
             if (P.count) {
                 const int bp = ok ? pix : -1;
-                if (P.bin_mode == BIN_PER_RAY) {
+                if (bin_mode == BIN_PER_RAY) {
                     if (bp >= 0) red_add(P.count + bp, 1);
                 } else {
                     // thread-local run-combine: consecutive rays of a thread mostly share a pixel
                     const bool flush = (bp != run_pix);
-                    flush_run(P, sh, run_pix, run_n, flush && run_pix >= 0);
+                    flush_run(P, sh, bin_mode, run_pix, run_n, flush && run_pix >= 0);
                     if (flush) { run_pix = bp; run_n = 1; } else { ++run_n; }
                 }
             }
         }
-        if (P.count && P.bin_mode != BIN_PER_RAY) flush_run(P, sh, run_pix, run_n, run_pix >= 0);
+        if (P.count && bin_mode != BIN_PER_RAY) flush_run(P, sh, bin_mode, run_pix, run_n, run_pix >= 0);
         n_in = __reduce_add_sync(0xffffffffu, n_in);
         n_out = __reduce_add_sync(0xffffffffu, n_out);
         n_lost = __reduce_add_sync(0xffffffffu, n_lost);
@@ -413,7 +415,7 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             if (n_lost) atomicAdd(&sh.ctr[2], (unsigned long long)n_lost);
         }
         __syncthreads();  // all epilogues done: near list and window are complete
-        if (P.bin_mode == BIN_WINDOW && P.count) {
+        if (bin_mode == BIN_WINDOW && P.count) {
             for (int t = tid; t < kWin * kWin; t += kThreads) {
                 const int v = sh.win[t];
                 if (v) {
