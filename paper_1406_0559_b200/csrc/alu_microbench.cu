@@ -32,14 +32,14 @@ __device__ __forceinline__ float rcp_mufu(float x) {
     return r;
 }
 
-enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, FFMA2_FMUL, FFMA2_MUFU_INDEP, FFMA2_3PAIRS, FFMA2_UBCAST, FFMA_3REGS, SHARED_MIX, N_MIX };
+enum Mix { FFMA = 0, FFMA2, MUFU, FFMA_MUFU_41, KERNEL_MIX, PAIRED_MIX, DFMA, FADD2_ONLY, LDS128, FFMA2_FMUL, FFMA2_MUFU_INDEP, FFMA2_3PAIRS, FFMA2_UBCAST, FFMA_3REGS, SHARED_MIX, KERNEL_NOMUFU, N_MIX };
 static const char* kMixName[N_MIX] = {"ffma", "ffma2", "mufu_rcp", "ffma4_mufu1", "kernel_mix_6ffma2_2mufu",
                                       "paired_mix_6ffma2_3fmul_1mufu", "dfma", "fadd2", "lds128_broadcast",
                                       "ffma2x12_fmulx6", "ffma2x12_mufux4_independent",
                                       "ffma2_three_distinct_pairs", "ffma2_uniform_bcast_operand", "ffma_three_distinct_regs",
-                                      "shared_mix_12ffma2_3fmul2_2mufu_per_4rays"};
+                                      "shared_mix_12ffma2_3fmul2_2mufu_per_4rays", "kernel_mix_without_mufu_6_packed_per_pair"};
 // warp-instructions issued per inner iteration per thread, FP32 flops per iteration per thread
-static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains, 18, 16, kChains, kChains, kChains, 68};
+static const int kInstr[N_MIX] = {kChains, kChains, kChains, 20, 64, 80, kChains, kChains, kChains, 18, 16, kChains, kChains, kChains, 68, 48};
 
 template <int MIX>
 __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycles, float seed, float useed) {
@@ -107,6 +107,17 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
                 const float2 pi = __ffma2_rn(c2, dx, b2);
                 p[k] = __ffma2_rn(pr, rc, p[k]);
                 s2[k] = __ffma2_rn(pi, rc, s2[k]);
+            }
+        } else if (MIX == KERNEL_NOMUFU) {
+            // the FMA side of the production loop alone (r2 stands in for its reciprocal): 6 packed per ray pair
+#pragma unroll
+            for (int k = 0; k < kChains / 2; ++k) {
+                const float2 dx = __fadd2_rn(p[k], c2);
+                const float2 r2 = __ffma2_rn(dx, dx, b2);
+                const float2 pr = __ffma2_rn(b2, dx, c2);
+                const float2 pi = __ffma2_rn(c2, dx, b2);
+                p[k] = __ffma2_rn(pr, r2, p[k]);
+                s2[k] = __ffma2_rn(pi, r2, s2[k]);
             }
         } else if (MIX == PAIRED_MIX) {
             // one reciprocal per ray pair: rc = 1/(r2.x*r2.y); 1/r2.x = rc*r2.y, 1/r2.y = rc*r2.x
@@ -294,6 +305,7 @@ int main(int argc, char** argv) {
     run<FFMA2_UBCAST>(sms, ctas, out, cyc, false);
     run<FFMA_3REGS>(sms, ctas, out, cyc, false);
     run<SHARED_MIX>(sms, ctas, out, cyc, false);
+    run<KERNEL_NOMUFU>(sms, ctas, out, cyc, false);
     int* map;  // 4096^2 int32 = 64 MB (config 3's map; fits the 126 MB L2) and 16384^2 = 1 GB (larger than L2)
     for (int big = 0; big < 2; ++big) {
         const unsigned n_pix = big ? (1u << 28) : (1u << 24);
