@@ -255,7 +255,7 @@ def test_config_sub_blocks(ml, oracle, cfg_id):
     assert l1 <= max(4, TOL_L1 * tot["in_map"]), (l1, tot)
 
 
-@pytest.mark.parametrize("cfg_id", [3, 4, 5])
+@pytest.mark.parametrize("cfg_id", [2, 3, 4, 5])
 def test_full_map_invariants(ml, oracle, cfg_id):
     # the launch configuration bench.py times: whole lattice, default options
     cfg = fields.CONFIGS[cfg_id]
@@ -284,6 +284,25 @@ def test_full_map_invariants(ml, oracle, cfg_id):
     print(f"cfg{cfg_id}: full map {st['elapsed_ms']:.1f} ms, <mu>/mu_th = {mean_mu / cfg.mu_th:.4f}, max count {st['max_count']}")
     if cfg_id in (3, 5):
         assert abs(mean_mu / cfg.mu_th - 1) < 0.15
+
+
+def test_config_1_full_map_against_the_oracle(ml, oracle):
+    # the one BASELINE.json config whose whole lattice the oracle shoots in about a second: full-map L1, all counters
+    cfg = fields.CONFIGS[1]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        count, mag, st = h.shoot()
+        count = count.cpu().numpy().astype(np.int64)
+        mag = mag.cpu().numpy()
+        g = h.geometry
+    ref = oracle.shoot_block(*_args(cfg), xy, m)
+    rs = ref["stats"]
+    assert st["rays_total"] == rs["rays_total"] == g.n1 * g.n2
+    l1 = int(np.abs(count - ref["count"]).sum())
+    print(f"cfg1 full map: in_map {st['rays_in_map']} (oracle {rs['rays_in_map']}), L1 {l1}, lost {st['rays_lost']}")
+    assert l1 <= TOL_L1 * rs["rays_in_map"]
+    assert abs(st["rays_in_map"] - rs["rays_in_map"]) <= l1 and st["rays_lost"] == rs["rays_lost"]
+    assert np.array_equal(mag, oracle.magnification(count.astype(np.int32), g.n_avg))
 
 
 def test_plain_fp32_ablation_fails_the_tolerances(ml, oracle):
