@@ -379,6 +379,21 @@ def run_mpd(args):
             torch.cuda.synchronize()
             ms.append(e0.elapsed_time(e1))
         _, mst = h.mpd(count, n_bins, hist=hist)
+        # row f5 on the same map: mlens_index_map (max reduction + MPD + compaction + 16-bit map; synchronous) and decode
+        ims, dms = [], []
+        for _ in range(args.steps):
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            values, indexed = h.index_map(count)
+            ims.append(1e3 * (time.perf_counter() - t0))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            back = h.unindex_map(indexed, values.contiguous())
+            e1.record()
+            torch.cuda.synchronize()
+            dms.append(e0.elapsed_time(e1))
+        assert torch.equal(back, count)
     med = statistics.median(ms)
     nbytes = 4 * cfg.npix**2
     peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(
@@ -387,7 +402,11 @@ def run_mpd(args):
     print(json.dumps({"mode": "mpd", "config": args.config, "npix": cfg.npix, "n_bins": n_bins, "ms": ms, "ms_median": med,
                       "algorithmic_bytes": nbytes, "achieved_gbs": gbs, "peak_gbs": peak, "frac": gbs / peak if peak else None,
                       "note": "includes the memset of the bins and of the stats struct (stream-ordered, same events)",
-                      "map_stats": mst}), flush=True)
+                      "map_stats": mst,
+                      "index_map": {"n_distinct": int(values.numel()), "ms_median_host_clock": statistics.median(ims),
+                                    "unindex_ms_median": statistics.median(dms),
+                                    "algorithmic_bytes": 10 * cfg.npix**2,  # MPD pass 4 B + apply 4 B in + 2 B out per pixel
+                                    "unindex_gbs": 6 * cfg.npix**2 / (statistics.median(dms) * 1e-3) / 1e9}}), flush=True)
 
 
 def run_convolve(args):
