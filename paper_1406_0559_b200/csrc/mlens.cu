@@ -52,7 +52,7 @@ struct mlens {
     int device;
     int sm_count;
     float4* lens_dev;                  // (x, y, m, 0)
-    unsigned long long* counters_dev;  // in_map, outside, lost, total
+    unsigned long long* counters_dev;  // in_map, outside, lost, total, [4] dynamic tile counter of the shooting kernel
     int* max_count_dev;
     mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
     mlk::MapStatsDev* mapstats_host;   // pinned mirror
@@ -107,6 +107,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     }
     P.count = count; P.ray_y = ray_y; P.ray_pix = ray_pix;
     P.counters = h->counters_dev;
+    MLENS_CUDA(cudaMemsetAsync(h->counters_dev + 4, 0, sizeof(unsigned long long), st));  // dynamic tile counter
     P.bin_mode = h->opt_binning;
 
     if (h->opt_kernel == 0) {
@@ -254,8 +255,8 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
     if (e == cudaSuccess && n_lens > 0)
         e = cudaMemcpy(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&h->counters_dev, 4 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&h->counters_dev, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, 8 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&h->max_count_dev, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(h->max_count_dev, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&h->counters_host, 8 * sizeof(unsigned long long));

@@ -19,7 +19,7 @@
 #include <stdint.h>
 
 #ifndef MLENS_HOT_UNROLL
-#define MLENS_HOT_UNROLL 24  // lenses per unrolled hot-loop iteration; measured best of {1,2,4,6,8,12,16,24} (profiles/r1c_summary.md)
+#define MLENS_HOT_UNROLL 16  // lenses per unrolled hot-loop iteration; re-swept after every change of the surrounding code
 #endif
 
 namespace mlk {
@@ -55,7 +55,7 @@ struct ShootParams {
     int* count;                     // npix*npix or nullptr
     double* ray_y;                  // optional per-ray outputs
     int* ray_pix;
-    unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total
+    unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total [4] dynamic tile counter (zeroed per launch)
     int bin_mode;
 };
 
@@ -96,6 +96,20 @@ __device__ __forceinline__ float rcp_mufu(float x) {
     return r;
 }
 
+// XU-free conversions for the per-ray epilogue.  F2F.F64.F32, I2F.F64 and F2I.F64 execute on the XU pipe — the pipe
+// the hot loop's MUFU.RCP saturates — at 16 clk per warp instruction; ~100 of them per warp and tile were the whole
+// per-tile fixed cost of the kernel (6 % of the run at N* = 430).  These run on the integer and FP64 pipes instead.
+//   f32_to_f64_bits: exact widening of a FINITE float by re-biasing the exponent (0 maps to 2^-127, harmless as an
+//                    addend; inf/NaN map to finite values, so finiteness must be tested on the float beforehand).
+//   floor_to_int:    floor(u) for 0 <= u < 2^31 via a round-down FP64 add of 2^52 + 2^51 (the integer lands in the low
+//                    mantissa word).
+__device__ __forceinline__ double f32_to_f64_bits(float x) {
+    const unsigned b = __float_as_uint(x);
+    const unsigned hi = (b & 0x80000000u) | (((b & 0x7fffffffu) >> 3) + 0x38000000u);
+    return __hiloint2double((int)hi, (int)(b << 29));
+}
+__device__ __forceinline__ int floor_to_int(double u) { return __double2loint(__dadd_rd(u, 6755399441055744.0)); }
+
 // ---------------------------------------------------------------------------------------------------------------
 // binning helpers (step a4)
 // ---------------------------------------------------------------------------------------------------------------
@@ -121,6 +135,7 @@ struct __align__(16) TileShared {
     double near_zx[kNearMax], near_zy[kNearMax], near_m[kNearMax];
     int near_n;
     int win_ix0, win_iy0;                    // binning window origin (BIN_WINDOW)
+    long long next_tile;                     // the CTA's next tile, fetched from the global counter by thread 0
     unsigned long long ctr[3];               // CTA-private ray counters
     int win[kWin * kWin];                    // CTA-private count window (BIN_WINDOW)
 };
@@ -181,6 +196,7 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
         dxb[j].y = (float)(((double)(tx * kR + 2 * j + 1) - 31.5) * P.d);
     }
 
+    const double dxt0 = (double)(tx * kR) - 31.5;  // in-tile offset of the thread's first ray, in lattice steps
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
     long long g = 0;  // sequence number of the raw-chunk load being consumed: buffer g&1, barrier phase (g>>1)&1
 
@@ -191,7 +207,15 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
         bulk_copy_g2s(raw0, P.lens_raw, bytes, &sh.bar[0]);
     }
 
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    // DYNAMIC tile scheduling.  Tiles are equal work, but the warp scheduler favours the older of an SM's two CTAs: with a
+    // static split the older one finished its share after ~65 % of the kernel and the other ran the rest alone, with its
+    // per-tile bookkeeping exposed (alone: 84 % of the paired rate at N* = 430, 92 % at N* = 2333).  Every CTA takes its
+    // first tile by index and every further one from a global counter, fetched one tile ahead by thread 0 so that the
+    // atomic's latency is hidden; all CTAs now finish within one tile of each other.  (Which CTA shoots a tile does not
+    // affect its arithmetic, and the map is built from integer REDs, so the result is unchanged.)
+    long long nxt = 0;  // thread 0 only
+    for (long long tile = blockIdx.x; tile < n_tiles;) {
+        if (tid == 0) nxt = (long long)atomicAdd(&P.counters[4], 1ull) + gridDim.x;
         const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
         const long long ti0 = P.i0 + (long long)tI * kTile, tj0 = P.j0 + (long long)tJ * kTile;
         const double Zcx = ((double)(ti0 + kTile / 2) - P.half_n1) * P.d;
@@ -247,7 +271,7 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
             if (P.n_chunks > 1 && tid == 0) {
                 int cn = c + 1;
                 long long tn = tile;
-                if (cn == P.n_chunks) { cn = 0; tn = tile + gridDim.x; }
+                if (cn == P.n_chunks) { cn = 0; tn = nxt; }
                 if (tn < n_tiles) {
                     const int nb = (int)((g + 1) & 1);
                     const uint32_t bytes = (uint32_t)min(P.chunk, P.n_lens - cn * P.chunk) * 16u;
@@ -336,6 +360,10 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
         const bool special = n_near > 0 || near_overflow;  // tile-uniform: near-lens list or FP64 fallback in play
         const bool want_rays = P.ray_y != nullptr || P.ray_pix != nullptr;
         const double npix_d = (double)P.npix;
+        // u1 of ray k = B1 + k*s1 + (delta*S)_re / p  with the thread's first in-tile offset folded into B1
+        const double s1 = P.f1 * P.d * P.inv_p;
+        const double B1 = fma(dxt0, s1, U1c);
+        const double B2 = fma(row2, P.inv_p, U2c);
 
 #pragma unroll
         for (int k = 0; k < kR; ++k) {
@@ -348,9 +376,9 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im);  y1 = f1 x1 - alpha1,  y2 = f2 x2 - alpha2
             const float ds_re = dxf * srf - dyf * sif;
             const float ds_im = dxf * sif + dyf * srf;
-            const double dxt = ((double)(tx * kR + k) - 31.5) * P.d;
-            double u1 = fma(fma(P.f1, dxt, (double)ds_re), P.inv_p, U1c);
-            double u2 = fma(row2 - (double)ds_im, P.inv_p, U2c);
+            double u1 = fma(f32_to_f64_bits(ds_re), P.inv_p, fma((double)k, s1, B1));
+            double u2 = fma(-f32_to_f64_bits(ds_im), P.inv_p, B2);
+            bool finite = fabsf(ds_re) <= 3.4028234663852886e38f && fabsf(ds_im) <= 3.4028234663852886e38f;
             if (special) {
                 const double dxd = (double)dxf;
                 double al1 = Acr - (double)ds_re;
@@ -376,12 +404,13 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
                 }
                 u1 = (P.f1 * x1 - al1 + P.half_L) * P.inv_p;
                 u2 = (P.f2 * x2 - al2 + P.half_L) * P.inv_p;
+                finite = fabs(u1) <= 1.7976931348623157e308 && fabs(u2) <= 1.7976931348623157e308;
             }
             int pix;
-            if (!(fabs(u1) <= 1.7976931348623157e308 && fabs(u2) <= 1.7976931348623157e308)) {
+            if (!finite) {
                 pix = -2;  // non-finite source position (ray on a lens): lost
             } else if (u1 >= 0.0 && u1 < npix_d && u2 >= 0.0 && u2 < npix_d) {
-                pix = (int)u2 * P.npix + (int)u1;  // u >= 0: truncation is floor
+                pix = floor_to_int(u2) * P.npix + floor_to_int(u1);
             } else {
                 pix = -1;
             }
@@ -424,8 +453,9 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
                 }
             }
         }
-        if (tid == 0) sh.near_n = 0;
+        if (tid == 0) { sh.near_n = 0; sh.next_tile = nxt; }
         __syncthreads();
+        tile = sh.next_tile;
     }
 
     if (tid == 0) {
