@@ -32,9 +32,27 @@ def build_microbench(force: bool = False) -> str:
     return MICRO_OUT
 
 
+PROBE_SRC = os.path.join(_HERE, "csrc", "umma_probe.cu")
+PROBE_OUT = os.path.join(_HERE, "lib", "umma_probe")
+
+
+def build_umma_probe(force: bool = False) -> str:
+    """The tensor-pipe probe for the next kernel generation; not on the product path."""
+    os.makedirs(os.path.dirname(PROBE_OUT), exist_ok=True)
+    if force or not os.path.exists(PROBE_OUT) or os.path.getmtime(PROBE_OUT) < os.path.getmtime(PROBE_SRC):
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-o", PROBE_OUT, PROBE_SRC]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    return PROBE_OUT
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(os.path.dirname(OUT), exist_ok=True)
     build_microbench(force)
+    build_umma_probe(force)
     stale = force or not os.path.exists(OUT) or any(os.path.getmtime(OUT) < os.path.getmtime(d) for d in DEPS)
     if stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
