@@ -7,7 +7,7 @@ import sys
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "mlens.cu")
-DEPS = [SRC, os.path.join(_HERE, "csrc", "shoot_kernel.cuh"), os.path.join(_HERE, "csrc", "mapstats_kernel.cuh"), os.path.join(_HERE, "csrc", "convolve_kernel.cuh"),
+DEPS = [SRC, os.path.join(_HERE, "csrc", "shoot_kernel.cuh"), os.path.join(_HERE, "csrc", "mapstats_kernel.cuh"), os.path.join(_HERE, "csrc", "convolve_kernel.cuh"), os.path.join(_HERE, "csrc", "shoot_umma_kernel.cuh"),
         os.path.join(os.path.dirname(_HERE), "include", "mlens.h")]
 OUT = os.path.join(_HERE, "lib", "libmlens.so")
 

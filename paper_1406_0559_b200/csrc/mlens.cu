@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdint>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -16,6 +17,7 @@
 #include "convolve_kernel.cuh"
 #include "mapstats_kernel.cuh"
 #include "shoot_kernel.cuh"
+#include "shoot_umma_kernel.cuh"
 
 namespace {
 
@@ -65,6 +67,7 @@ struct mlens {
     int* idx_lut;
     long long idx_bins_cap;
     int* idx_n_dev;
+    float* umma_A_dev;                 // kernel 3: ray matrix of one tile in UMMA layout (lazily built)
     unsigned int* mpd_partial;         // sm_count x kMpdSmemBinsMax per-CTA histogram slices (lazily allocated)
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
@@ -116,6 +119,35 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         const long long cap = (long long)h->sm_count * 16;
         if (blocks > cap) blocks = cap;
         mlk::shoot_fp64_kernel<<<(unsigned)blocks, 256, 0, st>>>(P);
+        MLENS_CUDA(cudaGetLastError());
+        return MLENS_OK;
+    }
+
+    if (h->opt_kernel == 3) {  // experimental: pre-reciprocal terms from the tensor pipe (shoot_umma_kernel.cuh)
+        if (!h->umma_A_dev) {
+            std::vector<float> A((size_t)mlk::kUmBlocks * mlk::kUmRays * 8, 0.f);
+            auto tf32 = [](float x) { uint32_t b; memcpy(&b, &x, 4); b = (b + 0x1000u) & 0xffffe000u; memcpy(&x, &b, 4); return x; };
+            for (int rb = 0; rb < mlk::kUmBlocks; ++rb)
+                for (int r = 0; r < mlk::kUmRays; ++r) {
+                    const double dx = (r % mlk::kTile) - 31.5, dy = (2 * rb + r / mlk::kTile) - 31.5;
+                    const double q = (dx * dx + dy * dy) * h->d * h->d;
+                    const float qh = tf32((float)q), ql = tf32((float)(q - (double)qh));
+                    const float row[8] = {1.f, 1.f, (float)dx, (float)dx, (float)dy, (float)dy, qh, ql};
+                    for (int k = 0; k < 8; ++k)
+                        A[((size_t)rb * mlk::kUmABlockBytes + mlk::umma_off_bytes(r, k)) / 4] = row[k];
+                }
+            MLENS_CUDA(cudaMalloc(&h->umma_A_dev, A.size() * sizeof(float)));
+            MLENS_CUDA(cudaMemcpyAsync(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+            MLENS_CUDA(cudaStreamSynchronize(st));
+        }
+        P.umma_A = h->umma_A_dev;
+        const size_t smem = (size_t)mlk::kUmBlocks * mlk::kUmABlockBytes + (size_t)(mlk::kUmSuper / mlk::kUmLenses) * mlk::kUmChunkBytes +
+                            (size_t)mlk::kTile * mlk::kTile * sizeof(float2) + sizeof(mlk::UmmaShared) + 1024;
+        const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
+        long long grid = h->sm_count;
+        if (grid > n_tiles) grid = n_tiles;
+        MLENS_CUDA(cudaFuncSetAttribute(mlk::shoot_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        mlk::shoot_umma_kernel<<<(unsigned)grid, mlk::kUmThreads, smem, st>>>(P);
         MLENS_CUDA(cudaGetLastError());
         return MLENS_OK;
     }
@@ -281,6 +313,7 @@ void mlens_destroy(mlens_t* h) {
     if (h->mapstats_dev) cudaFree(h->mapstats_dev);
     if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
     if (h->mpd_partial) cudaFree(h->mpd_partial);
+    if (h->umma_A_dev) cudaFree(h->umma_A_dev);
     if (h->idx_hist) cudaFree(h->idx_hist);
     if (h->idx_lut) cudaFree(h->idx_lut);
     if (h->idx_n_dev) cudaFree(h->idx_n_dev);
@@ -308,7 +341,7 @@ int mlens_get_geometry(const mlens_t* h, mlens_geometry* g) {
 int mlens_set_option(mlens_t* h, const char* key, long long value) {
     if (!h || !key) return fail(MLENS_EINVAL, "NULL argument");
     if (!strcmp(key, "kernel")) {
-        if (value < 0 || value > 2) return fail(MLENS_EINVAL, "kernel must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(MLENS_EINVAL, "kernel must be 0..3");
         h->opt_kernel = (int)value;
     } else if (!strcmp(key, "binning")) {
         if (value < 0 || value > 3) return fail(MLENS_EINVAL, "binning must be 0..3");

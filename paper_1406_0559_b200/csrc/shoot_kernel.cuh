@@ -57,6 +57,7 @@ struct ShootParams {
     int* ray_pix;
     unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total [4] dynamic tile counter (zeroed per launch)
     int bin_mode;
+    const float* umma_A;            // kernel 3 only: the 32 ray blocks of a tile in UMMA layout (shoot_umma_kernel.cuh)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
