@@ -104,6 +104,10 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
     const uint32_t tmem_base = sh.tmem_base;
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(kUmN >> 3) << 17) | ((uint32_t)(kUmRays >> 4) << 24);
 
+    // Ping-pong of the arithmetic phase between the two consumer groups (named barriers 1 and 2, 512 threads each):
+    // a group may only do its MUFU/FMA work while the other one waits for / reads its next accumulator, so the two can
+    // never fall into lock-step (both computing, then both waiting, with the MUFU idle a third of the time).
+    if (!is_control && (warp >> 3) == 1) asm volatile("bar.arrive 1, 512;" ::: "memory");
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
     const int n_super = P.n_lens > 0 ? (P.n_lens + kUmSuper - 1) / kUmSuper : 0;
     uint32_t seq = 0;  // MMA sequence number: buffer seq & 1, use (seq >> 1) of that buffer; same count in every warp
@@ -210,6 +214,10 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
                             tmem_ld16(tbase + kUmLenses + l16 * 32, pq);
                             tmem_ld16(tbase + kUmLenses + l16 * 32 + 16, pq + 16);
                             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                            if (hf == 0) {
+                                if (group == 0) asm volatile("bar.sync 1, 512;" ::: "memory");
+                                else asm volatile("bar.sync 2, 512;" ::: "memory");
+                            }
                             if (hf == 1) {
                                 // everything of this buffer is in registers: hand it back before the arithmetic
                                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -229,6 +237,8 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
                                 S[3] = __ffma2_rn(make_float2(pq[2 * j + 6], pq[2 * j + 7]), make_float2(RCb.y, RCb.y), S[3]);
                             }
                         }
+                        if (group == 0) asm volatile("bar.arrive 2, 512;" ::: "memory");
+                        else asm volatile("bar.arrive 1, 512;" ::: "memory");
                     }
                     const int ray = rb * kUmRays + quad * 32 + lane;
                     atomicAdd(&sS[ray].x, (S[0].x + S[1].x) + (S[2].x + S[3].x));
