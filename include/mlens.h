@@ -173,7 +173,7 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream);
  *               2 = ABLATION: plain-form FP32 kernel (does NOT meet the parity tolerances; <= 12000 lenses),
  *               3 = EXPERIMENTAL: second-generation kernel — r^2, Re, Im of every interaction from the tensor pipe (one
  *                   tcgen05 TF32 MMA per 128 rays x 64 lenses, accumulators in TMEM), shared reciprocals; meets the parity
- *                   tolerances, currently ~10 % slower than kernel 1 (pipeline bubbles between tensor pipe and MUFU)
+ *                   tolerances, currently ~10 % slower than kernel 1 (bound by TMEM read bandwidth: 12 B per interaction)
  *   "binning"   0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
  *               3 = + CTA-private shared-memory window
  *   "ctas_per_sm"  persistent CTAs per SM (default 2)
