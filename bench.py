@@ -13,6 +13,10 @@ another.  One JSON line is printed by rank 0.
                arrays in, count + magnification maps out), copies inside the timed region.
 * `roofline`   the shooting kernel alone: 11 flops x interactions / kernel time (events inside libmlens around the
                kernel launch) against the FP32 peak SMs x 128 x 2 x f_max; bound = "alu".
+               `peak_measured` / `frac_of_measured`: the scalar-FFMA rate measured on this box just before the timed
+               region by bench/alu_microbench --fp32-peak (MEASURED_PEAKS.json holds no FP32 figure), with the SM clock
+               observed inside that kernel.  `traffic`: DRAM bytes of one launch from the tracked ncu capture named in
+               `traffic_source` (null when no capture of the committed kernel exists for the workload).
 * `cpu_baseline` the FP64 oracle (oracle/) on the box's host cores on a bounded block of the same lattice.
 * N > 1        weak scaling: every rank shoots an independent map of the same config (seed + rank), the way the paper
                scales (one map per GPU); no data-path collective.
@@ -178,6 +182,78 @@ def run_reference(args):
 
 
 # -----------------------------------------------------------------------------------------------------------------
+# roofline inputs that are measured, not derived
+# -----------------------------------------------------------------------------------------------------------------
+def measure_fp32_peak(device_index: int):
+    """Scalar-FFMA rate of this GPU, measured now (bench/alu_microbench --fp32-peak, ~0.1 s).  None if it is not built."""
+    exe = os.path.join(ROOT, "bench", "alu_microbench")
+    if not os.path.exists(exe):
+        return None
+    try:
+        r = subprocess.run([exe, "--fp32-peak", str(device_index)], capture_output=True, text=True, timeout=120)
+        return json.loads(r.stdout.strip().splitlines()[-1]) if r.returncode == 0 else None
+    except (OSError, ValueError, IndexError, subprocess.TimeoutExpired):
+        return None
+
+
+def load_traffic(cfg_id: int, shard: bool):
+    """DRAM bytes (read + write) of ONE shooting-kernel launch of this workload from the tracked ncu capture of the
+    committed kernel, profiles/traffic_shoot_cfg<N>.json ({"dram_bytes_read", "dram_bytes_write", "command", ...}), or
+    (None, reason).  Never a literal in this file: the number and the command that produced it live under profiles/."""
+    if shard:
+        return None, "not captured for the sharded launch"
+    path = os.path.join(ROOT, "profiles", f"traffic_shoot_cfg{cfg_id}.json")
+    if not os.path.exists(path):
+        return None, f"no ncu capture of the committed kernel for config {cfg_id} under profiles/"
+    t = json.load(open(path))
+    return int(t["dram_bytes_read"]) + int(t["dram_bytes_write"]), f"profiles/traffic_shoot_cfg{cfg_id}.json ({t.get('command', '')})"
+
+
+def make_line(*, cfg_id, cfg, n_lens, n1, n2, world, shard, steps, warmup, ms_total, kern_ms, in_map, clocks, sms,
+              e2e_s, e2e_steps, h2d_bytes, d2h_bytes, peak_meas=None, traffic=None, traffic_source=None):
+    """The bench JSON line from the measured numbers (pure function: tests/test_bench_contract.py checks the contract)."""
+    rays = n1 * n2
+    inter = rays * max(1, n_lens)
+    f_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak = sms * FP32_LANES_PER_SM * 2 * f_max_mhz * 1e6 / 1e12  # TFLOP/s at the maximum SM clock
+    fpi = flops_per_interaction(cfg)
+    # shard mode: each rank's kernel covers 1/world of the interactions (kern_ms then also holds the all-reduce)
+    achieved = fpi * (inter / (world if shard else 1)) / (kern_ms * 1e-3) / 1e12
+    maps = 1 if shard else world
+    roof = {"bound": "alu", "kernel": "shoot_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
+            "algorithmic_bytes": 4 * cfg.npix**2 + 16 * n_lens,  # the count map written once + the lens list read once
+            "flops_per_interaction": fpi, "kernel_ms": kern_ms,
+            "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 x {f_max_mhz:.0f} MHz (clocks.max.sm); "
+                           "no FP32 figure in MEASURED_PEAKS.json",
+            "mufu_ceiling_frac": 16.0 * fpi / (FP32_LANES_PER_SM * 2)}
+    if peak_meas:
+        roof.update(peak_measured=peak_meas["fp32_tflops"], frac_of_measured=achieved / peak_meas["fp32_tflops"],
+                    peak_measured_sm_mhz=peak_meas.get("sm_mhz_observed"),
+                    peak_measured_source="bench/alu_microbench --fp32-peak on this GPU just before the timed region: "
+                                         + peak_meas.get("how", ""))
+    return {
+        "metric": METRIC, "value": maps * inter * steps / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps,
+        "warmup": warmup, "ms_per_step": ms_total / max(1, steps), "higher_is_better": True,
+        "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg_id, cfg, n_lens, n1, n2), "rays_per_map": rays,
+                   "interactions_per_map": inter, "rays_in_map": in_map,
+                   "mean_mu_over_mu_th": in_map / (cfg.npix**2 * cfg.sub**2) / cfg.mu_th,
+                   "l2": "256 MiB device write between steps (inputs are smaller than L2)",
+                   "parallelism": (f"one map, {world} row bands + one int32 all-reduce" if shard else
+                                   f"{world} independent map(s), one per GPU (seed + rank)")},
+        "rays_per_s": maps * rays * steps / (ms_total * 1e-3),
+        "clocks": clocks,
+        "e2e": {"value": maps * inter * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
+                "h2d_bytes_per_step": int(h2d_bytes), "d2h_bytes_per_step": int(d2h_bytes)},
+        # our kernels launched inside the timed region, by construction of mlens_shoot: one shooting kernel and one
+        # magnification kernel per step (the memsets are driver operations; the L2 flush is torch's fill)
+        "gpu_launches": 2 * steps,
+        "roofline": roof,
+    }
+
+
+# -----------------------------------------------------------------------------------------------------------------
 # our arm
 # -----------------------------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -233,6 +309,9 @@ def run_ours(args):
     for _ in range(args.warmup):
         step()
     barrier()
+    # measured FP32 peak of THIS box, taken after the warm-up (clocks ramped) and before the timed region (rank 0's GPU)
+    peak_meas = measure_fp32_peak(local_rank) if rank == 0 else None
+    barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
@@ -276,38 +355,12 @@ def run_ours(args):
 
     if rank == 0:
         prop = torch.cuda.get_device_properties(local_rank)
-        sms = prop.multi_processor_count
-        f_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
-        peak = sms * FP32_LANES_PER_SM * 2 * f_max_mhz * 1e6 / 1e12  # TFLOP/s at the maximum SM clock
-        fpi = flops_per_interaction(cfg)
-        # shard mode: each rank's kernel covers 1/world of the interactions (kern_ms then also holds the all-reduce)
-        achieved = fpi * (inter / (world if shard else 1)) / (kern_ms * 1e-3) / 1e12
-        maps = 1 if shard else world
-        value = maps * inter * args.steps / (ms_total * 1e-3)
-        # DRAM bytes of one shoot_fp32_kernel launch of the default workload (config 4, whole lattice), from
-        # profiles/r1_traffic_cfg4_full.csv (dram__bytes_read.sum + dram__bytes_write.sum); other workloads: not captured
-        traffic = 5098752 + 806948096 if (args.config == 4 and not shard) else None
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total / max(1, args.steps), "higher_is_better": True, "scaling": "strong" if shard else "weak",
-            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(args.config, cfg0, n_lens, g.n1, g.n2), "rays_per_map": rays,
-                       "interactions_per_map": inter, "rays_in_map": in_map,
-                       "l2": "256 MiB device write between steps (inputs are smaller than L2)",
-                       "parallelism": (f"one map, {world} row bands + one int32 all-reduce" if shard else
-                                       f"{world} independent map(s), one per GPU (seed + rank)")},
-            "rays_per_s": maps * rays * args.steps / (ms_total * 1e-3),
-            "clocks": clocks,
-            "e2e": {"value": maps * inter * e2e_steps / e2e_s, "unit": UNIT, "steps": e2e_steps,
-                    "h2d_bytes_per_step": int(xy.nbytes + m.nbytes), "d2h_bytes_per_step": int(c_host.nbytes + m_host.nbytes)},
-            "gpu_launches": 2 * args.steps,  # shoot_fp32_kernel + magnification_kernel per step (memsets are driver ops)
-            "roofline": {"bound": "alu", "kernel": "shoot_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": traffic, "flops_per_interaction": fpi,
-                         "kernel_ms": kern_ms,
-                         "peak_source": f"derived: {sms} SMs x 128 FP32 lanes x 2 x {f_max_mhz:.0f} MHz (clocks.max.sm); "
-                                        "no FP32 figure in MEASURED_PEAKS.json",
-                         "mufu_ceiling_frac": 16.0 * fpi / (FP32_LANES_PER_SM * 2)},
-        }
+        traffic, traffic_source = load_traffic(args.config, shard)
+        line = make_line(cfg_id=args.config, cfg=cfg0, n_lens=n_lens, n1=g.n1, n2=g.n2, world=world, shard=shard,
+                         steps=args.steps, warmup=args.warmup, ms_total=ms_total, kern_ms=kern_ms, in_map=in_map,
+                         clocks=clocks, sms=prop.multi_processor_count, e2e_s=e2e_s, e2e_steps=e2e_steps,
+                         h2d_bytes=xy.nbytes + m.nbytes, d2h_bytes=c_host.nbytes + m_host.nbytes, peak_meas=peak_meas,
+                         traffic=traffic, traffic_source=traffic_source)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = run_cpu_baseline(cfg, xy, m)
         print(json.dumps(line), flush=True)
@@ -324,7 +377,7 @@ def run_block(args):
     torch.cuda.set_device(0)
     cfg = fields.CONFIGS[args.config]
     xy, m = fields.lens_field(cfg)
-    with mlens.Mlens.from_config(cfg, xy, m) as h:
+    with mlens.Mlens.from_config(cfg, xy, m, ablations=args.ablations) as h:
         for k, v in (args.option or []):
             h.set_option(k, int(v))
         g = h.geometry
@@ -463,6 +516,7 @@ def main():
     ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
     ap.add_argument("--mpd", action="store_true", help="profile mode: time mlens_mpd on the config's shot map")
     ap.add_argument("--convolve", action="store_true", help="profile mode: time mlens_convolve on a map of the config's size")
+    ap.add_argument("--ablations", action="store_true", help="block mode: load libmlens_ablations.so (kernel / loop variants)")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
     args = ap.parse_args()
     if args.mpd:

@@ -6,7 +6,10 @@
 // the wall time from CUDA events (their ratio is the SM frequency during the run).
 //
 // Build:  nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -o alu_microbench alu_microbench.cu
-// Run:    ./alu_microbench            (prints one JSON object)
+//         (paper_1406_0559_b200/build.py: build_microbench(); not part of libmlens.so)
+// Run:    ./alu_microbench              every mix + the RED patterns (prints one JSON object)
+//         ./alu_microbench --fp32-peak [device]  the scalar-FFMA rate alone, ~0.1 s: the MEASURED FP32 peak bench.py reports
+//                                       beside the derived one ("measure it ... and report the clock")
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -68,6 +71,8 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
 #pragma unroll
     for (int k = 0; k < kChains; ++k) { xs[k] = xx[k >> 1].x + k; ys[k] = yy[k >> 1].y - k; }
     const float2 u2 = make_float2(useed, useed);  // kernel parameter: lives in a uniform register
+    unsigned long long g0 = 0, g1 = 0;
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
     const long long t0 = clock64();
     for (int it = 0; it < kIters; ++it) {
         if (MIX == FFMA) {
@@ -188,13 +193,17 @@ __global__ void __launch_bounds__(256) bench_kernel(float* out, long long* cycle
         }
     }
     const long long t1 = clock64();
+    if (threadIdx.x == 0) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     float s = 0.f;
 #pragma unroll
     for (int k = 0; k < kChains; ++k) s += a[k] + (float)dd[k];
 #pragma unroll
     for (int k = 0; k < kChains / 2; ++k) s += p[k].x + p[k].y + s2[k].x + s2[k].y + xx[k].x + yy[k].y;
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+    if (threadIdx.x == 0) {
+        cycles[blockIdx.x] = t1 - t0;
+        if (blockIdx.x == 0) cycles[gridDim.x] = (long long)(g1 - g0);  // ns on the global timer over the same span
+    }
 }
 
 template <int MIX>
@@ -279,16 +288,51 @@ void run_red(const char* name, int sms, int* map, unsigned mask, bool last) {
            last ? "" : ",");
 }
 
+// --fp32-peak: scalar FFMA, 16 independent chains per thread, 4 CTAs x 256 threads per SM (8 warps per SMSP), best of
+// 10 launches after a 20-launch warm-up (clock ramp).  flops = 2 per FFMA lane.  The SM clock is observed INSIDE the
+// timed kernel: CTA 0's clock64() span over its %globaltimer span.
+static int fp32_peak(int sms, float* out, long long* cyc) {
+    const int grid = sms * 4;
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    for (int w = 0; w < 20; ++w) bench_kernel<FFMA><<<grid, 256>>>(out, cyc, 1.0f, 0.5f);
+    CK(cudaDeviceSynchronize());
+    float best = 1e30f;
+    double mhz = 0.0;
+    for (int rep = 0; rep < 10; ++rep) {
+        CK(cudaEventRecord(e0));
+        bench_kernel<FFMA><<<grid, 256>>>(out, cyc, 1.0f, 0.5f);
+        CK(cudaEventRecord(e1));
+        CK(cudaEventSynchronize(e1));
+        float ms;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        long long c0, ns;
+        CK(cudaMemcpy(&c0, cyc, sizeof(c0), cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(&ns, cyc + grid, sizeof(ns), cudaMemcpyDeviceToHost));
+        if (ms < best) { best = ms; mhz = ns > 0 ? 1e3 * (double)c0 / (double)ns : 0.0; }
+    }
+    const double flops = 2.0 * (double)kIters * kChains * 256.0 * grid;
+    printf("{\"fp32_tflops\": %.4f, \"ms\": %.4f, \"sm_mhz_observed\": %.1f, \"sms\": %d, "
+           "\"how\": \"scalar FFMA, 16 chains/thread, 4x256 threads/SM, best of 10, CUDA events\"}\n",
+           flops / (best * 1e-3) / 1e12, best, mhz, sms);
+    return 0;
+}
+
 int main(int argc, char** argv) {
-    int ctas = argc > 1 ? atoi(argv[1]) : 4;
+    const bool peak_only = argc > 1 && !strcmp(argv[1], "--fp32-peak");
+    int ctas = (argc > 1 && !peak_only) ? atoi(argv[1]) : 4;
+    const int dev = (peak_only && argc > 2) ? atoi(argv[2]) : 0;
+    CK(cudaSetDevice(dev));
     cudaDeviceProp prop;
-    CK(cudaGetDeviceProperties(&prop, 0));
+    CK(cudaGetDeviceProperties(&prop, dev));
     const int sms = prop.multiProcessorCount;
     g_clock_hz = 1e3 * (double)prop.clockRate;
     float* out;
     long long* cyc;
     CK(cudaMalloc(&out, sizeof(float) * sms * 8 * 256));
-    CK(cudaMalloc(&cyc, sizeof(long long) * sms * 8));
+    CK(cudaMalloc(&cyc, sizeof(long long) * (sms * 8 + 1)));
+    if (peak_only) return fp32_peak(sms, out, cyc);
     printf("{\n  \"device\": \"%s\", \"sms\": %d, \"clock_rate_khz\": %d,\n", prop.name, sms, prop.clockRate);
     run<FFMA>(sms, ctas, out, cyc, false);
     run<FFMA2>(sms, ctas, out, cyc, false);

@@ -19,8 +19,17 @@
  * Every function returns MLENS_OK (0) or a negative mlens_status; none throws or aborts.  After a failure
  * mlens_last_error() returns a thread-local description.  There is NO CPU fallback: without a CUDA device
  * mlens_create fails with MLENS_ECUDA.  Pointers are marked HOST or DEVICE; DEVICE pointers must belong to the device
- * that was current when mlens_create was called.  `cuda_stream` is a cudaStream_t passed as void* (NULL = the
- * legacy default stream).  Calls on one handle must not be issued concurrently from several host threads.
+ * that was current when mlens_create was called, and that device must be the calling thread's current device in every
+ * later call on the handle (checked: MLENS_EINVAL otherwise).  DEVICE map pointers (count, mag, hist, indexed, values,
+ * kernel, out) must be 16-byte aligned — the kernels use 128-bit accesses; any cudaMalloc'ed or torch-allocated buffer
+ * is.  `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *
+ * Concurrency.  Calls on one handle must not be issued concurrently from several host threads.  From ONE thread:
+ *   - mlens_shoot_block launches of one handle MAY be issued to different streams and overlap on the device: each
+ *     launch owns its tile counter (up to 256 launches in flight), the ray counters and the count map are atomic sums;
+ *   - mlens_shoot, mlens_mpd, mlens_index_map, mlens_profile_kernel and mlens_convolve use per-handle scratch (events,
+ *     histogram slices, spectra, cuFFT plans): calls of these on one handle must be ordered after one another — issue
+ *     them to one stream, or order the streams with events.  Use one handle per stream for concurrent maps.
  */
 #ifndef MLENS_H_
 #define MLENS_H_
@@ -168,18 +177,18 @@ int mlens_get_stats(mlens_t* h, void* cuda_stream, mlens_stats* stats);
 /* Zero the device ray counters (asynchronous). */
 int mlens_reset_stats(mlens_t* h, void* cuda_stream);
 
-/* Tuning / ablation switches.  Keys:
- *   "kernel"    0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 1 = FP32 difference-form kernel (default),
- *               2 = ABLATION: plain-form FP32 kernel (does NOT meet the parity tolerances; <= 12000 lenses),
- *               3 = EXPERIMENTAL: second-generation kernel — r^2, Re, Im of every interaction from the tensor pipe (one
- *                   tcgen05 TF32 MMA per 128 rays x 64 lenses, accumulators in TMEM), shared reciprocals; meets the parity
- *                   tolerances, currently ~10 % slower than kernel 1 (bound by TMEM read bandwidth: 12 B per interaction)
- *   "binning"   0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
- *               3 = + CTA-private shared-memory window
+/* Tuning switches.  Keys of the shipped library (libmlens.so):
+ *   "binning"      0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
+ *                  3 = + CTA-private shared-memory window — four routes to the same map, bit-identical results
  *   "ctas_per_sm"  persistent CTAs per SM (default 2)
- *   "shared_rcp"   how many of a thread's 4-ray groups per lens take their four reciprocals from TWO MUFU.RCP of packed
- *                  products (0 = one MUFU.RCP per interaction); at most rays_per_thread/4
- *   "rays_per_thread"  8 (512-thread CTAs, default) or 16 (256-thread CTAs); the tile is 64 x 64 rays either way
+ *   "kernel"       1 = the production FP32 difference-form kernel (the only value the shipped library accepts)
+ * The debug / ablation / experimental kernels are compiled only with -DMLENS_ABLATIONS (libmlens_ablations.so, which
+ * the tests and profiling runs load; the shipped library returns MLENS_EINVAL for them, so the public ABI cannot
+ * select a kernel that misses the parity tolerances):
+ *   "kernel"       0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 2 = plain-form FP32 kernel (does NOT meet
+ *                  the parity tolerances: the evidence for the difference form; <= 12000 lenses), 3 = tensor-pipe
+ *                  experiment (r^2, Re, Im of every interaction from tcgen05 TF32 MMAs; slower than kernel 1)
+ *   "shared_rcp", "rays_per_thread"   loop variants of kernel 1
  * Returns MLENS_EINVAL for an unknown key or value. */
 int mlens_set_option(mlens_t* h, const char* key, long long value);
 

@@ -117,15 +117,18 @@ def shoot_rays(kappa, gamma, s, L, npix, d, lens_xy, lens_m, ray_ij, n_threads=0
     return {"y": y, "alpha": al, "scale": sc, "pix": pix}
 
 
-def map_points(kappa, gamma, s, lens_xy, lens_m, x):
-    """Eq. (1) at arbitrary image-plane positions x (n, 2) float64.  Returns (y, alpha)."""
+def map_points(kappa, gamma, s, lens_xy, lens_m, x, want_scale=False):
+    """Eq. (1) at arbitrary image-plane positions x (n, 2) float64.  Returns (y, alpha) or, with ``want_scale``,
+    (y, alpha, scale) where scale = sum_i m_i/|x - x_i| (the north_star's deflection-tolerance scale)."""
     xy, m, n = _lens(lens_xy, lens_m)
     x = np.ascontiguousarray(np.asarray(x, dtype=np.float64).reshape(-1, 2))
     y = np.empty_like(x); al = np.empty_like(x)
+    sc = np.empty((x.shape[0],), dtype=np.float64) if want_scale else None
     lib().oracle_map_points(ctypes.c_double(kappa), ctypes.c_double(gamma), ctypes.c_double(s), _p(xy, ctypes.c_float),
                             _p(m, ctypes.c_float), ctypes.c_longlong(n), _p(x, ctypes.c_double),
-                            ctypes.c_longlong(x.shape[0]), _p(y, ctypes.c_double), _p(al, ctypes.c_double))
-    return y, al
+                            ctypes.c_longlong(x.shape[0]), _p(y, ctypes.c_double), _p(al, ctypes.c_double),
+                            _p(sc, ctypes.c_double))
+    return (y, al, sc) if want_scale else (y, al)
 
 
 def pixels_of(y, L, npix):

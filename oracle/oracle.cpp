@@ -24,9 +24,11 @@
 //   S16 mag = (float)((double)count / N_avg)
 //
 // Pins (tests/test_oracle_pins.py, -m "not gpu"): P1 no-lens closed form, P2 single point lens A(u), P3 hand sums
-// (tests/golden/p3_hand_sums.txt), P4 ray conservation, P5 mean magnification, P6 mirror symmetry, P7 lens-order
-// permutation, P8 mass-sheet transformation.  Parity status: pinned (the dense many-caustic regime itself has no
-// closed form; there this code path, anchored by P1-P8, is the reference).
+// incl. the tolerance scale sum m/|x - x_i| (tests/golden/p3_hand_sums.txt), P4 ray conservation, P5 mean
+// magnification, P6 mirror symmetry, P7 lens-order permutation, P8 mass-sheet transformation, P14 per-ray outputs of
+// oracle_shoot_block / oracle_shoot_rays (y, alpha, scale, pixel) against oracle_map_points at lattice positions the
+// TEST computes from reading S2, and against each other.  Parity status: pinned (the dense many-caustic regime itself
+// has no closed form; there this code path, anchored by P1-P8 and P14, is the reference).
 //
 // Build: g++ -O3 -march=native -fopenmp -shared -fPIC oracle/oracle.cpp -o oracle/liboracle.so   (no fast-math)
 
@@ -92,6 +94,10 @@ static inline void shoot_one(double x1, double x2, double kappa_s, double gamma,
     if (scale) *scale = sc;
 }
 
+// Image-plane position of lattice index k along an axis with n rays (reading S2): cell-centred, symmetric about 0.
+// The ONE place the lattice formula is written; oracle_shoot_block and oracle_shoot_rays both call it.
+static inline double lattice_x(long long k, long long n, double d) { return ((double)k + 0.5 - (double)n / 2.0) * d; }
+
 // Pixel id of a source position: >= 0 in map, -1 outside, -2 non-finite (readings S4, S7).
 static inline int pixel_of(double y1, double y2, double L, double p, int npix) {
     if (!std::isfinite(y1) || !std::isfinite(y2)) return -2;
@@ -118,9 +124,9 @@ int oracle_shoot_block(double kappa, double gamma, double s, double L, int npix,
 #endif
 #pragma omp parallel for schedule(dynamic, 1) reduction(+ : in_map, outside, lost)
     for (long long jj = 0; jj < nj; ++jj) {
-        const double x2 = ((double)(j0 + jj) + 0.5 - (double)g.n2 / 2.0) * d;
+        const double x2 = lattice_x(j0 + jj, g.n2, d);
         for (long long ii = 0; ii < ni; ++ii) {
-            const double x1 = ((double)(i0 + ii) + 0.5 - (double)g.n1 / 2.0) * d;
+            const double x1 = lattice_x(i0 + ii, g.n1, d);
             double y1, y2, al1, al2, sc = 0.0;
             shoot_one(x1, x2, g.kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, ray_scale ? &sc : nullptr);
             const int pix = pixel_of(y1, y2, L, g.p, npix);
@@ -162,8 +168,8 @@ int oracle_shoot_rays(double kappa, double gamma, double s, double L, int npix, 
 #endif
 #pragma omp parallel for schedule(dynamic, 64)
     for (long long q = 0; q < n_rays; ++q) {
-        const double x1 = ((double)ray_ij[2 * q] + 0.5 - (double)g.n1 / 2.0) * d;
-        const double x2 = ((double)ray_ij[2 * q + 1] + 0.5 - (double)g.n2 / 2.0) * d;
+        const double x1 = lattice_x(ray_ij[2 * q], g.n1, d);
+        const double x2 = lattice_x(ray_ij[2 * q + 1], g.n2, d);
         double y1, y2, al1, al2, sc = 0.0;
         shoot_one(x1, x2, g.kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, ray_scale ? &sc : nullptr);
         if (ray_y) { ray_y[2 * q] = y1; ray_y[2 * q + 1] = y2; }
@@ -175,14 +181,17 @@ int oracle_shoot_rays(double kappa, double gamma, double s, double L, int npix, 
 }
 
 // Arbitrary image-plane positions (not lattice rays): used by pin P3 (hand sums, Appendix D of SURVEY.md).
+// scale (optional): the per-ray tolerance scale sum_i m_i/|x - x_i| of the same shoot_one call.
 int oracle_map_points(double kappa, double gamma, double s, const float* lens_xy, const float* lens_m,
-                      long long n_lens, const double* x, long long n_pts, double* y, double* alpha) {
+                      long long n_lens, const double* x, long long n_pts, double* y, double* alpha, double* scale) {
     const double kappa_s = s * kappa;
     for (long long q = 0; q < n_pts; ++q) {
-        double y1, y2, al1, al2;
-        shoot_one(x[2 * q], x[2 * q + 1], kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2, nullptr);
+        double y1, y2, al1, al2, sc = 0.0;
+        shoot_one(x[2 * q], x[2 * q + 1], kappa_s, gamma, lens_xy, lens_m, n_lens, &y1, &y2, &al1, &al2,
+                  scale ? &sc : nullptr);
         y[2 * q] = y1; y[2 * q + 1] = y2;
         if (alpha) { alpha[2 * q] = al1; alpha[2 * q + 1] = al2; }
+        if (scale) scale[q] = sc;
     }
     return 0;
 }

@@ -17,7 +17,9 @@
 #include "convolve_kernel.cuh"
 #include "mapstats_kernel.cuh"
 #include "shoot_kernel.cuh"
+#ifdef MLENS_ABLATIONS
 #include "shoot_umma_kernel.cuh"
+#endif
 
 namespace {
 
@@ -41,6 +43,7 @@ int fail(int code, const char* fmt, ...) {
 
 constexpr int kChunkMax = 2048;        // lenses per chunk when the list is streamed in several chunks
 constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chunk
+constexpr int kTileCtrSlots = 256;     // ring of dynamic tile counters: one per launch in flight (see launch_block)
 
 }  // namespace
 
@@ -54,7 +57,9 @@ struct mlens {
     int device;
     int sm_count;
     float4* lens_dev;                  // (x, y, m, 0)
-    unsigned long long* counters_dev;  // in_map, outside, lost, total, [4] dynamic tile counter of the shooting kernel
+    unsigned long long* counters_dev;  // in_map, outside, lost, total
+    unsigned long long* tile_ctr_dev;  // ring of kTileCtrSlots dynamic tile counters; launch number n uses slot n % kTileCtrSlots
+    unsigned long long launch_seq;
     int* max_count_dev;
     mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
     mlk::MapStatsDev* mapstats_host;   // pinned mirror
@@ -82,7 +87,16 @@ struct mlens {
 
 namespace {
 
-int check_handle(const mlens_t* h) { return h ? MLENS_OK : fail(MLENS_EINVAL, "NULL handle"); }
+// NULL handle, or a handle whose device is not the calling thread's current device (its buffers, plans and the
+// caller's DEVICE pointers all belong to h->device: launching from another device would fault or silently misbehave)
+int check_handle(const mlens_t* h) {
+    if (!h) return fail(MLENS_EINVAL, "NULL handle");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(MLENS_ECUDA, "cudaGetDevice failed");
+    if (dev != h->device)
+        return fail(MLENS_EINVAL, "current CUDA device is %d but the handle was created on device %d", dev, h->device);
+    return MLENS_OK;
+}
 
 int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long nj, int* count, double* ray_y,
                  int* ray_pix, cudaStream_t st) {
@@ -110,9 +124,14 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     }
     P.count = count; P.ray_y = ray_y; P.ray_pix = ray_pix;
     P.counters = h->counters_dev;
-    MLENS_CUDA(cudaMemsetAsync(h->counters_dev + 4, 0, sizeof(unsigned long long), st));  // dynamic tile counter
+    // Every launch gets its OWN dynamic tile counter, zeroed on the launch's stream: launches of one handle issued to
+    // different streams may then overlap without stealing or re-zeroing each other's tiles (the ray counters are
+    // plain atomic sums and do not care).  A slot is reused after kTileCtrSlots further launches.
+    P.tile_counter = h->tile_ctr_dev + (h->launch_seq++ % kTileCtrSlots);
+    MLENS_CUDA(cudaMemsetAsync(P.tile_counter, 0, sizeof(unsigned long long), st));
     P.bin_mode = h->opt_binning;
 
+#ifdef MLENS_ABLATIONS
     if (h->opt_kernel == 0) {
         const long long n_rays = ni * nj;
         long long blocks = (n_rays + 255) / 256;
@@ -137,8 +156,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
                         A[((size_t)rb * mlk::kUmABlockBytes + mlk::umma_off_bytes(r, k)) / 4] = row[k];
                 }
             MLENS_CUDA(cudaMalloc(&h->umma_A_dev, A.size() * sizeof(float)));
-            MLENS_CUDA(cudaMemcpyAsync(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice, st));
-            MLENS_CUDA(cudaStreamSynchronize(st));
+            MLENS_CUDA(cudaMemcpy(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice));
         }
         P.umma_A = h->umma_A_dev;
         const size_t smem = (size_t)mlk::kUmBlocks * mlk::kUmABlockBytes + (size_t)(mlk::kUmSuper / mlk::kUmLenses) * mlk::kUmChunkBytes +
@@ -164,6 +182,8 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         return MLENS_OK;
     }
 
+#endif  // MLENS_ABLATIONS
+
     int chunk, n_chunks;
     if (P.n_lens <= kChunkSingleMax) {
         chunk = (P.n_lens + 3) & ~3;
@@ -182,8 +202,11 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     const int code = h->opt_rays * 100 + h->opt_shared;
     switch (code) {
 #define MLENS_VARIANT(R, SH) case R * 100 + SH: kern = mlk::shoot_fp32_kernel<R, SH, -1>; break;
+        MLENS_VARIANT(8, 0)
+#ifdef MLENS_ABLATIONS
         MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
-        MLENS_VARIANT(8, 0) MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2)
+        MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2)
+#endif
 #undef MLENS_VARIANT
         default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d shared_rcp=%d", h->opt_rays, h->opt_shared);
     }
@@ -261,7 +284,12 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     g.n2 = 2 * (long long)c2;
     g.n_avg = (g.p / ray_spacing) * (g.p / ray_spacing);
 
-    std::vector<float4> packed((size_t)n_lens);
+    std::vector<float4> packed;
+    try {
+        packed.resize((size_t)n_lens);
+    } catch (...) {  // nothing may throw across the C ABI
+        return fail(MLENS_ENOMEM, "host allocation of %lld lenses failed", n_lens);
+    }
     for (long long k = 0; k < n_lens; ++k) {
         const float x = lens_xy[2 * k], y = lens_xy[2 * k + 1], m = lens_m ? lens_m[k] : 1.0f;
         if (!std::isfinite(x) || !std::isfinite(y)) return fail(MLENS_EINVAL, "lens %lld has a non-finite coordinate", k);
@@ -273,7 +301,7 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     MLENS_CUDA(cudaGetDevice(&dev));
     cudaDeviceProp prop;
     MLENS_CUDA(cudaGetDeviceProperties(&prop, dev));
-    if (prop.major < 10) return fail(MLENS_ECUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
+    if (prop.major != 10) return fail(MLENS_ECUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
 
     mlens* h = new (std::nothrow) mlens();
     if (!h) return fail(MLENS_ENOMEM, "host allocation failed");
@@ -289,6 +317,7 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
         e = cudaMemcpy(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&h->counters_dev, 8 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&h->tile_ctr_dev, kTileCtrSlots * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMalloc(&h->max_count_dev, sizeof(int));
     if (e == cudaSuccess) e = cudaMemset(h->max_count_dev, 0, sizeof(int));
     if (e == cudaSuccess) e = cudaMallocHost(&h->counters_host, 8 * sizeof(unsigned long long));
@@ -309,6 +338,7 @@ void mlens_destroy(mlens_t* h) {
     if (!h) return;
     if (h->lens_dev) cudaFree(h->lens_dev);
     if (h->counters_dev) cudaFree(h->counters_dev);
+    if (h->tile_ctr_dev) cudaFree(h->tile_ctr_dev);
     if (h->max_count_dev) cudaFree(h->max_count_dev);
     if (h->mapstats_dev) cudaFree(h->mapstats_dev);
     if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
@@ -340,6 +370,13 @@ int mlens_get_geometry(const mlens_t* h, mlens_geometry* g) {
 
 int mlens_set_option(mlens_t* h, const char* key, long long value) {
     if (!h || !key) return fail(MLENS_EINVAL, "NULL argument");
+#ifndef MLENS_ABLATIONS
+    // the shipped library holds the production kernel only: the debug / ablation / experimental kernels and loop variants
+    // exist in the MLENS_ABLATIONS build (libmlens_ablations.so, used by the tests and the profiling runs)
+    if ((!strcmp(key, "kernel") && value != 1) || (!strcmp(key, "shared_rcp") && value != 0) ||
+        (!strcmp(key, "rays_per_thread") && value != 8))
+        return fail(MLENS_EINVAL, "option %s=%lld needs the MLENS_ABLATIONS build of the library", key, value);
+#endif
     if (!strcmp(key, "kernel")) {
         if (value < 0 || value > 3) return fail(MLENS_EINVAL, "kernel must be 0..3");
         h->opt_kernel = (int)value;
@@ -369,6 +406,7 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream) {
 
 int mlens_get_stats(mlens_t* h, void* cuda_stream, mlens_stats* stats) {
     if (!h || !stats) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     return read_stats(h, (cudaStream_t)cuda_stream, stats);
 }
 
@@ -383,12 +421,14 @@ int mlens_shoot_block(mlens_t* h, long long i0, long long j0, long long ni, long
 
 int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* cuda_stream) {
     if (!h || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     return launch_magnification(h, count_dev, mag_dev, (cudaStream_t)cuda_stream);
 }
 
 int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, int n_bins, void* cuda_stream,
               mlens_map_stats* stats) {
     if (!h || !count_dev || !hist_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     if (n_bins < 2) return fail(MLENS_EINVAL, "n_bins must be >= 2");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (!h->mapstats_dev) MLENS_CUDA(cudaMalloc(&h->mapstats_dev, sizeof(mlk::MapStatsDev)));
@@ -428,6 +468,7 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
 int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_values, unsigned short* indexed_dev,
                     void* cuda_stream, int* n_distinct) {
     if (!h || !count_dev || !values_dev || !indexed_dev || !n_distinct) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     if (max_values < 1) return fail(MLENS_EINVAL, "max_values must be >= 1");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long n = (long long)h->npix * h->npix;
@@ -438,6 +479,7 @@ int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_v
     int max_count;
     memcpy(&max_count, h->counters_host + 4, sizeof(int));
     const long long n_bins = (long long)max_count + 2;
+    if (n_bins > 2147483647LL) return fail(MLENS_ERANGE, "largest count %d: the histogram would need more than 2^31-1 bins", max_count);
     if (n_bins > h->idx_bins_cap) {
         if (h->idx_hist) cudaFree(h->idx_hist);
         if (h->idx_lut) cudaFree(h->idx_lut);
@@ -471,6 +513,7 @@ int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_v
 int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* values_dev, int n_values, int* count_dev,
                       void* cuda_stream) {
     if (!h || !indexed_dev || !values_dev || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     if (n_values < 1 || n_values > 65536) return fail(MLENS_EINVAL, "n_values must be 1..65536");
     const long long n = (long long)h->npix * h->npix;
     long long blocks = (n / 4 + 255) / 256;
@@ -483,6 +526,7 @@ int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* 
 
 int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kernel_dev, void* cuda_stream) {
     if (!h || !kernel_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     if (shape != mlk::PROFILE_UNIFORM_DISC && shape != mlk::PROFILE_GAUSSIAN) return fail(MLENS_EINVAL, "unknown profile shape %d", shape);
     if (!std::isfinite(size_pixels) || !(size_pixels > 0)) return fail(MLENS_EINVAL, "profile size must be finite and > 0");
     const double half = shape == mlk::PROFILE_GAUSSIAN ? std::ceil(4.0 * size_pixels) : std::ceil(size_pixels);
@@ -513,6 +557,7 @@ int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kerne
 
 int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, float* out_dev, void* cuda_stream) {
     if (!h || !map_dev || !kernel_dev || !out_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int N = h->npix;
     const long long nc = (long long)N * (N / 2 + 1);  // complex elements of an R2C spectrum
@@ -540,6 +585,7 @@ int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, fl
 
 int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, mlens_stats* stats) {
     if (!h || !count_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t n = (size_t)h->npix * h->npix;
     if (stats) MLENS_CUDA(cudaEventRecord(h->ev0, st));
@@ -561,6 +607,7 @@ int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, m
 
 int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* stats) {
     if (!h || !count_host) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
     const size_t n = (size_t)h->npix * h->npix;
     if (!h->own_stream) MLENS_CUDA(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
     if (!h->count_own) MLENS_CUDA(cudaMalloc(&h->count_own, n * sizeof(int)));

@@ -55,7 +55,8 @@ struct ShootParams {
     int* count;                     // npix*npix or nullptr
     double* ray_y;                  // optional per-ray outputs
     int* ray_pix;
-    unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total [4] dynamic tile counter (zeroed per launch)
+    unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total
+    unsigned long long* tile_counter;  // this launch's dynamic tile counter (zeroed on the launch's stream)
     int bin_mode;
     const float* umma_A;            // kernel 3 only: the 32 ray blocks of a tile in UMMA layout (shoot_umma_kernel.cuh)
 };
@@ -216,7 +217,7 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
     // affect its arithmetic, and the map is built from integer REDs, so the result is unchanged.)
     long long nxt = 0;  // thread 0 only
     for (long long tile = blockIdx.x; tile < n_tiles;) {
-        if (tid == 0) nxt = (long long)atomicAdd(&P.counters[4], 1ull) + gridDim.x;
+        if (tid == 0) nxt = (long long)atomicAdd(P.tile_counter, 1ull) + gridDim.x;
         const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
         const long long ti0 = P.i0 + (long long)tI * kTile, tj0 = P.j0 + (long long)tJ * kTile;
         const double Zcx = ((double)(ti0 + kTile / 2) - P.half_n1) * P.d;
@@ -332,7 +333,6 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
         const long long jray = tj0 + ty;
         const bool row_ok = jray < P.j0 + P.nj;
         const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
-        const double dyd = (double)dyf;
         int n_in = 0, n_out = 0, n_lost = 0;
         int run_pix = -1, run_n = 0;
 
@@ -381,11 +381,13 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
             double u2 = fma(-f32_to_f64_bits(ds_im), P.inv_p, B2);
             bool finite = fabsf(ds_re) <= 3.4028234663852886e38f && fabsf(ds_im) <= 3.4028234663852886e38f;
             if (special) {
-                const double dxd = (double)dxf;
+                // exact FP64 in-tile offsets here: the float-rounded ones are off by ~1e-9 R_E, which a ray 1e-4 R_E from
+                // a lens (deflection gradient m/r^2 ~ 1e8) turns into tens of pixels
+                const double dxd = (dxt0 + (double)k) * P.d;
                 double al1 = Acr - (double)ds_re;
                 double al2 = -(Aci - (double)ds_im);
                 for (int q = 0; q < n_near; ++q) {
-                    const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyd;
+                    const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyt;
                     const double f = sh.near_m[q] / (wx * wx + wy * wy);
                     al1 += f * wx;
                     al2 += f * wy;
@@ -468,6 +470,7 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
     }
 }
 
+#ifdef MLENS_ABLATIONS
 // ---------------------------------------------------------------------------------------------------------------
 // ABLATION ONLY (mlens_set_option("kernel", 2)): the "obvious" FP32 kernel — Eq. (1) summed in plain FP32 in global
 // coordinates, same tiling, register blocking, packed arithmetic and MUFU reciprocal as the production kernel but no
@@ -596,6 +599,8 @@ __global__ void __launch_bounds__(256) shoot_fp64_kernel(const ShootParams P) {
         if (n_in + n_out + n_lost) atomicAdd(&P.counters[3], (unsigned long long)(n_in + n_out + n_lost));
     }
 }
+
+#endif  // MLENS_ABLATIONS
 
 // ---------------------------------------------------------------------------------------------------------------
 // step a5 (Eq. 4): mag = (float)((double)count / N_avg); HBM-bound, 8 B per pixel

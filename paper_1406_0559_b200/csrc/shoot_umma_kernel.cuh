@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
     uint32_t seq = 0;  // MMA sequence number: buffer seq & 1, use (seq >> 1) of that buffer; same count in every warp
     long long nxt = 0;
     for (long long tile = blockIdx.x; tile < n_tiles;) {
-        if (tid == 0) nxt = (long long)atomicAdd(&P.counters[4], 1ull) + gridDim.x;
+        if (tid == 0) nxt = (long long)atomicAdd(P.tile_counter, 1ull) + gridDim.x;
         const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
         const long long ti0 = P.i0 + (long long)tI * kTile, tj0 = P.j0 + (long long)tJ * kTile;
         const double Zcx = ((double)(ti0 + kTile / 2) - P.half_n1) * P.d;

@@ -77,6 +77,12 @@ class MapConfig:
         return (h / abs(1.0 - self.kappa - self.gamma), h / abs(1.0 - self.kappa + self.gamma))
 
     @property
+    def map_half_image(self) -> tuple[float, float]:
+        """Half-widths of the map's pre-image under the macro-model alone: (L/2)/|1-kappa-+gamma| = half_widths/margin."""
+        a1, a2 = self.half_widths
+        return (a1 / self.margin, a2 / self.margin)
+
+    @property
     def disc_radius(self) -> float:
         a1, a2 = self.half_widths
         return self.margin * math.sqrt(a1 * a1 + a2 * a2)
@@ -159,11 +165,16 @@ def random_field(n: int, radius: float, seed: int, masses: str = "unit") -> tupl
 
 
 def block_plan(n1: int, n2: int, lens_xy: np.ndarray, half_widths: tuple[float, float], d: float, seed: int,
-               n_random: int = 32, n_lens_centred: int = 16, n_border: int = 8, size: int = 256) -> list[tuple[int, int, int, int]]:
+               n_random: int = 32, n_lens_centred: int = 16, n_border: int = 8, size: int = 256,
+               n_straddle: int = 0, n_inside: int = 0, map_half_image: tuple[float, float] | None = None
+               ) -> list[tuple[int, int, int, int]]:
     """Seeded (i0, j0, ni, nj) ray sub-blocks for parity at the large configs (SURVEY.md §8(d) sub-block plan).
 
-    Random unaligned blocks, blocks centred on lenses (near-lens path), blocks touching the lattice border.
-    Pure index bookkeeping: which rays to compare, not how they are shot.
+    Random unaligned blocks, blocks centred on lenses (near-lens path), blocks touching the lattice border, and — when
+    ``map_half_image`` = (b1, b2) is given — blocks that straddle / lie inside the image-plane rectangle |x1| < b1,
+    |x2| < b2 (the caller passes the pre-image of the map under the macro-model, b = (L/2)/|1-kappa-+gamma| =
+    half_width/margin: the region whose rays the macro-model alone would send into the map, so that the compared sample
+    holds in-map rays).  Pure index bookkeeping: which rays to compare, not how they are shot.
     """
     sx, sy = min(size, n1), min(size, n2)
     u = uniform01(seed ^ 0xB10C, 0, 4 * (n_random + n_lens_centred + n_border) + 8)
@@ -195,4 +206,28 @@ def block_plan(n1: int, n2: int, lens_xy: np.ndarray, half_widths: tuple[float, 
             blocks.append((n1 - sx, r, sx, sy))
         else:
             blocks.append((r, n2 - sy, sx, sy))
+    if (n_straddle or n_inside) and map_half_image is not None:
+        b1, b2 = map_half_image
+        v = uniform01(seed ^ 0x57AD, 0, 2 * (n_straddle + n_inside) + 2)
+        # lattice index of image-plane position x along an axis with n rays: x = (i + 1/2 - n/2) d
+        def idx(x, n):
+            return int(math.floor(x / d + n / 2.0))
+
+        def clamp(i0, n, sz):
+            return min(max(i0, 0), n - sz)
+
+        k = 0
+        for t in range(n_straddle):  # block centred on one of the four edges of the map's macro pre-image
+            r = 2.0 * v[k] - 1.0
+            k += 1
+            side = -1.0 if (t // 2) % 2 == 0 else 1.0
+            if t % 2 == 0:   # an edge x1 = +-b1, anywhere along it
+                ic, jc = idx(side * b1, n1), idx(0.9 * r * b2, n2)
+            else:            # an edge x2 = +-b2
+                ic, jc = idx(0.9 * r * b1, n1), idx(side * b2, n2)
+            blocks.append((clamp(ic - sx // 2, n1, sx), clamp(jc - sy // 2, n2, sy), sx, sy))
+        for t in range(n_inside):    # block well inside the pre-image (central 80 %)
+            ic, jc = idx(0.8 * (2.0 * v[k] - 1.0) * b1, n1), idx(0.8 * (2.0 * v[k + 1] - 1.0) * b2, n2)
+            k += 2
+            blocks.append((clamp(ic - sx // 2, n1, sx), clamp(jc - sy // 2, n2, sy), sx, sy))
     return blocks

@@ -13,7 +13,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "lib", "libmlens.so")
-_lib = None
+LIB_PATH_ABLATIONS = os.path.join(_HERE, "lib", "libmlens_ablations.so")  # -DMLENS_ABLATIONS build: tests / profiling only
+_libs: dict = {}
 
 OK, EINVAL, ENOMEM, ECUDA, ERANGE = 0, -1, -2, -3, -4
 
@@ -48,14 +49,18 @@ class MapStats(ctypes.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-def lib() -> ctypes.CDLL:
-    """Load libmlens.so and declare the prototypes of every symbol in include/mlens.h.  Raises if it is not built."""
-    global _lib
-    if _lib is not None:
-        return _lib
-    if not os.path.exists(LIB_PATH):
-        raise RuntimeError(f"{LIB_PATH} is missing: build it first (__graft_entry__.build()); there is no CPU fallback")
-    L = ctypes.CDLL(LIB_PATH)
+def lib(ablations: bool = False) -> ctypes.CDLL:
+    """Load libmlens.so and declare the prototypes of every symbol in include/mlens.h.  Raises if it is not built.
+
+    ``ablations=True`` loads libmlens_ablations.so instead: the same ABI compiled with -DMLENS_ABLATIONS, in which
+    ``mlens_set_option`` can also select the debug / ablation / experimental kernels (tests and profiling only)."""
+    key = bool(ablations)
+    if key in _libs:
+        return _libs[key]
+    path = LIB_PATH_ABLATIONS if key else LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it first (__graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(path)
     vp, ll, dbl, ci = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_double, ctypes.c_int
     L.mlens_create.argtypes = [ctypes.POINTER(vp), dbl, dbl, dbl, dbl, ci, dbl, vp, vp, ll]
     L.mlens_shoot.argtypes = [vp, vp, vp, vp, ctypes.POINTER(Stats)]
@@ -79,13 +84,13 @@ def lib() -> ctypes.CDLL:
                  "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
         getattr(L, name).restype = ci
-    _lib = L
+    _libs[key] = L
     return L
 
 
-def _check(rc: int):
+def _check(rc: int, L=None):
     if rc != 0:
-        raise MlensError(rc, lib().mlens_last_error().decode())
+        raise MlensError(rc, (L or lib()).mlens_last_error().decode())
 
 
 def _stream_ptr(stream=None):
@@ -98,8 +103,8 @@ def _stream_ptr(stream=None):
 class Mlens:
     """A map context: mlens_create ... mlens_destroy.  Device tensors are torch tensors on the current CUDA device."""
 
-    def __init__(self, kappa, gamma, s, map_side, npix, ray_spacing, lens_xy, lens_m=None):
-        L = lib()
+    def __init__(self, kappa, gamma, s, map_side, npix, ray_spacing, lens_xy, lens_m=None, ablations=False):
+        L = self._L = lib(ablations)
         xy = np.ascontiguousarray(np.asarray(lens_xy, dtype=np.float32).reshape(-1))
         m = None if lens_m is None else np.ascontiguousarray(np.asarray(lens_m, dtype=np.float32).reshape(-1))
         n = xy.size // 2
@@ -107,21 +112,24 @@ class Mlens:
             raise ValueError("lens_m and lens_xy disagree on the number of lenses")
         self._h = ctypes.c_void_p()
         self.npix = int(npix)
-        _check(L.mlens_create(ctypes.byref(self._h), kappa, gamma, s, map_side, int(npix), ray_spacing,
+        self._ck(L.mlens_create(ctypes.byref(self._h), kappa, gamma, s, map_side, int(npix), ray_spacing,
                               xy.ctypes.data_as(ctypes.c_void_p) if n else None,
                               m.ctypes.data_as(ctypes.c_void_p) if m is not None and n else None, n))
         g = Geometry()
-        _check(L.mlens_get_geometry(self._h, ctypes.byref(g)))
+        self._ck(L.mlens_get_geometry(self._h, ctypes.byref(g)))
         self.geometry = g
         self.n_lens = n
 
     @classmethod
-    def from_config(cls, cfg, lens_xy, lens_m):
-        return cls(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, lens_xy, lens_m)
+    def from_config(cls, cfg, lens_xy, lens_m, ablations=False):
+        return cls(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, lens_xy, lens_m, ablations)
+
+    def _ck(self, rc: int):
+        _check(rc, self._L)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:
-            lib().mlens_destroy(self._h)
+            self._L.mlens_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __del__(self):
@@ -137,7 +145,7 @@ class Mlens:
         self.close()
 
     def set_option(self, key: str, value: int):
-        _check(lib().mlens_set_option(self._h, key.encode(), int(value)))
+        self._ck(self._L.mlens_set_option(self._h, key.encode(), int(value)))
 
     # -- step a1-a5: the whole map -----------------------------------------------------------------------------
     def shoot(self, count=None, mag=None, want_mag=True, stream=None, sync=True):
@@ -151,7 +159,7 @@ class Mlens:
         assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
         assert mag is None or (mag.is_cuda and mag.dtype == torch.float32 and mag.is_contiguous() and mag.numel() == self.npix**2)
         st = Stats() if sync else None
-        _check(lib().mlens_shoot(self._h, ctypes.c_void_p(count.data_ptr()),
+        self._ck(self._L.mlens_shoot(self._h, ctypes.c_void_p(count.data_ptr()),
                                  ctypes.c_void_p(mag.data_ptr()) if mag is not None else None, _stream_ptr(stream),
                                  ctypes.byref(st) if sync else None))
         return count, mag, (st.as_dict() if sync else None)
@@ -167,7 +175,7 @@ class Mlens:
             pix = torch.empty((nj, ni), dtype=torch.int32, device="cuda")
         if count is not None:
             assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
-        _check(lib().mlens_shoot_block(self._h, int(i0), int(j0), int(ni), int(nj),
+        self._ck(self._L.mlens_shoot_block(self._h, int(i0), int(j0), int(ni), int(nj),
                                        ctypes.c_void_p(count.data_ptr()) if count is not None else None,
                                        ctypes.c_void_p(y.data_ptr()) if y is not None else None,
                                        ctypes.c_void_p(pix.data_ptr()) if pix is not None else None, _stream_ptr(stream)))
@@ -178,7 +186,7 @@ class Mlens:
         count = np.empty((self.npix, self.npix), dtype=np.int32)
         mag = np.empty((self.npix, self.npix), dtype=np.float32) if want_mag else None
         st = Stats()
-        _check(lib().mlens_shoot_host(self._h, count.ctypes.data_as(ctypes.c_void_p),
+        self._ck(self._L.mlens_shoot_host(self._h, count.ctypes.data_as(ctypes.c_void_p),
                                       mag.ctypes.data_as(ctypes.c_void_p) if mag is not None else None, ctypes.byref(st)))
         return count, mag, st.as_dict()
 
@@ -187,7 +195,7 @@ class Mlens:
 
         if mag is None:
             mag = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
-        _check(lib().mlens_magnification(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(mag.data_ptr()),
+        self._ck(self._L.mlens_magnification(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(mag.data_ptr()),
                                          _stream_ptr(stream)))
         return mag
 
@@ -201,7 +209,7 @@ class Mlens:
         assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous() and hist.numel() == int(n_bins)
         assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous() and count.numel() == self.npix**2
         ms = MapStats() if sync else None
-        _check(lib().mlens_mpd(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(hist.data_ptr()), int(n_bins),
+        self._ck(self._L.mlens_mpd(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(hist.data_ptr()), int(n_bins),
                                _stream_ptr(stream), ctypes.byref(ms) if sync else None))
         return hist, (ms.as_dict() if sync else None)
 
@@ -213,7 +221,7 @@ class Mlens:
         values = torch.empty((int(max_values),), dtype=torch.int32, device="cuda")
         indexed = torch.empty((self.npix, self.npix), dtype=torch.uint16, device="cuda")
         nd = ctypes.c_int(0)
-        _check(lib().mlens_index_map(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(values.data_ptr()),
+        self._ck(self._L.mlens_index_map(self._h, ctypes.c_void_p(count.data_ptr()), ctypes.c_void_p(values.data_ptr()),
                                      int(max_values), ctypes.c_void_p(indexed.data_ptr()), _stream_ptr(stream), ctypes.byref(nd)))
         return values[: nd.value], indexed
 
@@ -225,7 +233,7 @@ class Mlens:
             count = torch.empty((self.npix, self.npix), dtype=torch.int32, device="cuda")
         assert indexed.is_cuda and indexed.dtype == torch.uint16 and indexed.is_contiguous() and indexed.numel() == self.npix**2
         assert values.is_cuda and values.dtype == torch.int32 and values.is_contiguous()
-        _check(lib().mlens_unindex_map(self._h, ctypes.c_void_p(indexed.data_ptr()), ctypes.c_void_p(values.data_ptr()),
+        self._ck(self._L.mlens_unindex_map(self._h, ctypes.c_void_p(indexed.data_ptr()), ctypes.c_void_p(values.data_ptr()),
                                        int(values.numel()), ctypes.c_void_p(count.data_ptr()), _stream_ptr(stream)))
         return count
 
@@ -236,7 +244,7 @@ class Mlens:
         if kernel is None:
             kernel = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
         assert kernel.is_cuda and kernel.dtype == torch.float32 and kernel.is_contiguous() and kernel.numel() == self.npix**2
-        _check(lib().mlens_profile_kernel(self._h, int(shape), float(size_pixels), ctypes.c_void_p(kernel.data_ptr()),
+        self._ck(self._L.mlens_profile_kernel(self._h, int(shape), float(size_pixels), ctypes.c_void_p(kernel.data_ptr()),
                                           _stream_ptr(stream)))
         return kernel
 
@@ -249,14 +257,14 @@ class Mlens:
         for t in (mag, kernel, out):
             assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.npix**2
         assert out.data_ptr() not in (mag.data_ptr(), kernel.data_ptr())
-        _check(lib().mlens_convolve(self._h, ctypes.c_void_p(mag.data_ptr()), ctypes.c_void_p(kernel.data_ptr()),
+        self._ck(self._L.mlens_convolve(self._h, ctypes.c_void_p(mag.data_ptr()), ctypes.c_void_p(kernel.data_ptr()),
                                     ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
     def stats(self, stream=None):
         st = Stats()
-        _check(lib().mlens_get_stats(self._h, _stream_ptr(stream), ctypes.byref(st)))
+        self._ck(self._L.mlens_get_stats(self._h, _stream_ptr(stream), ctypes.byref(st)))
         return st.as_dict()
 
     def reset_stats(self, stream=None):
-        _check(lib().mlens_reset_stats(self._h, _stream_ptr(stream)))
+        self._ck(self._L.mlens_reset_stats(self._h, _stream_ptr(stream)))

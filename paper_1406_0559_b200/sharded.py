@@ -49,16 +49,21 @@ def allreduce_map(count, counters, group=None):
     return count, counters
 
 
-def shoot_sharded(h, rank: int, world: int, count=None, mag=None, want_mag=True, group=None, stream=None):
+def shoot_sharded(h, rank: int, world: int, count=None, mag=None, want_mag=True, group=None, stream=None, device="cuda"):
     """Shoot rank ``rank``'s row band of ``h``'s lattice, all-reduce the maps, then Eq. 4 on the summed map.
 
     ``h`` is a ``mlens.Mlens`` created with the SAME parameters and lens arrays on every rank.  Returns
-    (count, mag or None, stats dict) — identical on every rank.  ``stats['band']`` is this rank's (j0, nj)."""
+    (count, mag or None, stats dict) — identical on every rank.  ``stats['band']`` is this rank's (j0, nj).
+
+    Only five members of ``h`` are used — ``geometry`` (n1, n2), ``npix``, ``reset_stats``, ``shoot_block``, ``stats`` and
+    ``magnification`` — so the multi-process CPU test (tests/test_sharded.py, gloo, world_size 2) drives THIS function
+    with a stand-in handle whose band shooter is the oracle and ``device="cpu"``; the product always passes a
+    ``mlens.Mlens`` and CUDA tensors."""
     import torch
 
     g = h.geometry
     if count is None:
-        count = torch.empty((h.npix, h.npix), dtype=torch.int32, device="cuda")
+        count = torch.empty((h.npix, h.npix), dtype=torch.int32, device=device)
     count.zero_()
     h.reset_stats(stream)
     j0, nj = row_bands(g.n2, world)[rank]

@@ -32,3 +32,36 @@ def test_reference_arm_prints_one_contract_line():
 def test_reference_arm_other_ranks_are_silent():
     r = _run({"RANK": "1", "WORLD_SIZE": "2"})
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpu_arm_line_contract_from_measured_numbers():
+    # bench.make_line is the pure function that assembles the GPU arm's JSON line; fed here with made-up measurements
+    # for a 2-rank sharded run and a 1-rank run (the timing itself needs the B200 box)
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_1406_0559_b200 import fields
+
+    cfg = fields.CONFIGS[4]
+    kw = dict(cfg_id=4, cfg=cfg, n_lens=2333, n1=122880, n2=122880, steps=3, warmup=3, ms_total=3 * 8000.0, kern_ms=7990.0,
+              in_map=1_820_000_000, clocks={"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}, sms=148, e2e_s=16.2,
+              e2e_steps=2, h2d_bytes=28000, d2h_bytes=8 << 20)
+    one = bench.make_line(world=1, shard=False, peak_meas={"fp32_tflops": 71.8, "sm_mhz_observed": 1965.0, "how": "x"},
+                          traffic=4_500_000, traffic_source="profiles/x.json", **kw)
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline"):
+        assert key in one, key
+    inter = 122880 * 122880 * 2333
+    assert one["metric"] == "ray_lens_interactions_per_s" and one["scaling"] == "weak" and one["n_gpus"] == 1
+    assert abs(one["value"] / (inter / 8.0) - 1) < 1e-12 and one["ms_per_step"] == 8000.0 and one["vs_baseline"] is None
+    assert "workload" in one["config"] and "model" not in one["config"] and one["dtype"] == "f32"
+    r = one["roofline"]
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-15
+    assert abs(r["achieved"] - 11 * inter / 7.99 / 1e12) < 1e-9 and abs(r["peak"] - 148 * 128 * 2 * 1.965e9 / 1e12) < 1e-9
+    assert r["peak_measured"] == 71.8 and abs(r["frac_of_measured"] - r["achieved"] / 71.8) < 1e-15
+    assert r["traffic"] == 4_500_000 and r["traffic_source"] == "profiles/x.json"
+    assert one["e2e"]["h2d_bytes_per_step"] == 28000 and one["e2e"]["d2h_bytes_per_step"] == 8 << 20
+    two = bench.make_line(world=2, shard=True, **kw)
+    assert two["scaling"] == "strong" and two["n_gpus"] == 2 and "row bands" in two["config"]["parallelism"]
+    assert abs(two["value"] - one["value"]) < 1e-3  # ONE map on two GPUs: the job is the same map
+    assert abs(two["roofline"]["achieved"] * 2 - one["roofline"]["achieved"]) < 1e-9  # each rank shoots half of it
+    assert two["roofline"]["traffic"] is None and "peak_measured" not in two["roofline"]

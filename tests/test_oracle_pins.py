@@ -109,7 +109,7 @@ def _read_p3():
         elif t[0] == "lens":
             lenses.append([float(v) for v in t[1:4]])
         elif t[0] == "ray":
-            rays.append([float(Fraction(v)) for v in t[1:7]] + [int(t[7])])
+            rays.append([float(Fraction(v)) for v in t[1:7]] + [int(t[7])] + [float(Fraction(v)) for v in t[8:10]] + [float(t[10])])
     return params, np.array(lenses), np.array(rays)
 
 
@@ -123,6 +123,61 @@ def test_p3_hand_sums(oracle):
     assert np.abs(y - rays[:, 4:6]).max() <= 1e-14
     pix = oracle.pixels_of(y, prm["L"], int(prm["npix"]))
     assert pix.tolist() == rays[:, 6].astype(int).tolist()
+
+
+def test_p3_tolerance_scale_hand_sums(oracle):
+    # sum_i m_i/|x - x_i| — the bound of GPU parity check (i) — against the hand-worked column of the golden file.
+    # A dropped sqrt (m/r^2), a dropped mass or a squared mass each miss these values by >= 5 %.
+    prm, lenses, rays = _read_p3()
+    xy = lenses[:, :2].astype(np.float32)
+    m = lenses[:, 2].astype(np.float32)
+    y, alpha, scale = oracle.map_points(prm["kappa"], prm["gamma"], prm["s"], xy, m, rays[:, 0:2], want_scale=True)
+    assert np.abs(scale / rays[:, 9] - 1.0).max() <= 1e-14
+    # the golden column is consistent with the golden squared distances (guards the file itself against typos)
+    assert np.abs((1.0 / np.sqrt(rays[:, 7]) + 0.5 / np.sqrt(rays[:, 8])) / rays[:, 9] - 1.0).max() <= 1e-15
+    # and asking for the scale does not change y / alpha
+    y0, a0 = oracle.map_points(prm["kappa"], prm["gamma"], prm["s"], xy, m, rays[:, 0:2])
+    assert np.array_equal(y, y0) and np.array_equal(alpha, a0)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# P14 — the per-ray outputs the GPU parity tests consume (oracle_shoot_block / oracle_shoot_rays: y, alpha, scale, pixel)
+# ---------------------------------------------------------------------------------------------------------------
+def test_p14_per_ray_outputs_of_block_and_ray_list(oracle):
+    # Lattice positions are computed HERE from reading S2 (x = (i + 1/2 - n/2) d with n from the closed-form geometry
+    # numbers of SURVEY.md App. A) and pushed through oracle_map_points, which P3 pins to the hand sums.  An i/j mix-up,
+    # an off-by-half or a transposed (nj, ni) layout in either per-ray path fails: the block is not square, the lattice
+    # is not (n1 != n2) and the macro factors differ per axis.
+    cfg = fields.MapConfig("p14", 48, 3.0, 0.35, 0.15, 0.4, 3, "salpeter", 141)
+    xy, m = fields.random_field(17, cfg.disc_radius, 141, "salpeter")
+    args = (cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
+    d = cfg.ray_spacing
+    a1, a2 = 1.2 * 1.5 / abs(1 - 0.35 - 0.15), 1.2 * 1.5 / abs(1 - 0.35 + 0.15)
+    n1, n2 = 2 * math.ceil(a1 / d - 1e-9), 2 * math.ceil(a2 / d - 1e-9)
+    g = oracle.geometry(*args)
+    assert (g.n1, g.n2) == (n1, n2) and n1 != n2
+    i0, j0, ni, nj = 11, 5, 37, 23
+    blk = oracle.shoot_block(*args, xy, m, block=(i0, j0, ni, nj), want_rays=True)
+    ii, jj = np.meshgrid(np.arange(i0, i0 + ni), np.arange(j0, j0 + nj))          # [jj, ii] layout: row = j
+    x = np.stack([(ii + 0.5 - n1 / 2.0) * d, (jj + 0.5 - n2 / 2.0) * d], axis=-1)   # S2, written out
+    y, al, sc = oracle.map_points(cfg.kappa, cfg.gamma, cfg.s, xy, m, x.reshape(-1, 2), want_scale=True)
+    # (not bit equality: the compiler may contract a*b+c differently in the two inlined copies of the ray loop)
+    def close(a, b):
+        return np.abs(a - b).max() <= 1e-13 * (1.0 + np.abs(b).max())
+
+    assert close(blk["y"].reshape(-1, 2), y) and close(blk["alpha"].reshape(-1, 2), al)
+    assert close(blk["scale"].reshape(-1), sc) and sc.min() > 0
+    assert np.array_equal(blk["pix"].reshape(-1), oracle.pixels_of(y, cfg.map_side, cfg.npix))
+    # the same rays as an (i, j) list, in a shuffled order
+    ij = np.stack([ii.reshape(-1), jj.reshape(-1)], axis=1)
+    perm = np.argsort(fields.uniform01(5, 0, len(ij)))
+    lst = oracle.shoot_rays(*args, xy, m, ij[perm])
+    assert close(lst["y"], y[perm]) and close(lst["alpha"], al[perm])
+    assert close(lst["scale"], sc[perm]) and np.array_equal(lst["pix"], blk["pix"].reshape(-1)[perm])
+    # scale against its definition evaluated by numpy for a few rays (independent of shoot_one's loop)
+    for q in (0, 100, len(ij) - 1):
+        r = np.hypot(x.reshape(-1, 2)[q, 0] - xy[:, 0].astype(np.float64), x.reshape(-1, 2)[q, 1] - xy[:, 1].astype(np.float64))
+        assert abs(float((m.astype(np.float64) / r).sum()) / sc[q] - 1.0) <= 1e-13
 
 
 def test_p3_pixel_convention_edges(oracle):

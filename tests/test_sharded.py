@@ -39,9 +39,43 @@ def _free_port():
         return s.getsockname()[1]
 
 
+class _OracleHandle:
+    """Stand-in for ``mlens.Mlens`` on a box without a GPU: same five members ``shoot_sharded`` uses, CPU tensors, the
+    FP64 oracle as the band shooter.  Test infrastructure only."""
+
+    def __init__(self, oracle, cfg, xy, m):
+        self.o, self.cfg, self.xy, self.m = oracle, cfg, xy, m
+        self.args = (cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
+        self.geometry = oracle.geometry(*self.args)
+        self.npix = cfg.npix
+        self.ctr = dict(rays_total=0, rays_in_map=0, rays_outside=0, rays_lost=0)
+        self.max_count = -1
+        self.calls = []
+
+    def reset_stats(self, stream=None):
+        self.calls.append("reset")
+        for k in self.ctr:
+            self.ctr[k] = 0
+
+    def shoot_block(self, i0, j0, ni, nj, count=None, stream=None):
+        self.calls.append(("band", i0, j0, ni, nj))
+        c = count.numpy()  # shares memory with the tensor: accumulates in place, like the kernel
+        r = self.o.shoot_block(*self.args, self.xy, self.m, block=(i0, j0, ni, nj), count=c)
+        for k in self.ctr:
+            self.ctr[k] += r["stats"][k]
+
+    def stats(self, stream=None):
+        return dict(self.ctr, n_lens=len(self.m), max_count=self.max_count, elapsed_ms=0.0, kernel_ms=0.0)
+
+    def magnification(self, count, mag=None, stream=None):
+        self.calls.append("mag")
+        self.max_count = int(count.max())
+        return torch.from_numpy(self.o.magnification(count.numpy(), self.geometry.n_avg))
+
+
 def _gloo_worker(rank, world, port, q):
-    """Each rank shoots its band with the ORACLE (the CPU stand-in for the per-rank kernel launch), then the maps go
-    through the same allreduce_map the GPU path uses."""
+    """Every rank runs the REAL sharded.shoot_sharded (band plan, zeroing, counters tensor, both all-reduces, Eq. 4 on the
+    summed map, max_count refresh) on CPU tensors over gloo; only the per-band kernel launch is replaced by the oracle."""
     import oracle
 
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
@@ -49,34 +83,35 @@ def _gloo_worker(rank, world, port, q):
     try:
         cfg = dataclasses.replace(fields.CONFIGS[1], npix=64, sub=4)
         xy, m = fields.lens_field(cfg)
-        args = (cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
-        g = oracle.geometry(*args)
-        j0, nj = sharded.row_bands(g.n2, world)[rank]
-        r = oracle.shoot_block(*args, xy, m, block=(0, j0, g.n1, nj))
-        st = r["stats"]
-        count = torch.from_numpy(r["count"].astype(np.int32))
-        counters = torch.tensor([st["rays_in_map"], st["rays_outside"], st["rays_lost"], st["rays_total"]], dtype=torch.int64)
-        sharded.allreduce_map(count, counters)
-        if rank == 0:
-            full = oracle.shoot_block(*args, xy, m)
-            q.put((bool(np.array_equal(count.numpy(), full["count"])), counters.tolist(),
-                   [full["stats"][k] for k in ("rays_in_map", "rays_outside", "rays_lost", "rays_total")], g.n1 * g.n2))
+        h = _OracleHandle(oracle, cfg, xy, m)
+        count = torch.full((cfg.npix, cfg.npix), 7, dtype=torch.int32)  # stale contents: shoot_sharded must zero them
+        count, mag, st = sharded.shoot_sharded(h, rank, world, count=count, device="cpu")
+        full = oracle.shoot_block(*h.args, xy, m)
+        ok = bool(np.array_equal(count.numpy(), full["count"]))
+        ok_mag = bool(np.array_equal(mag.numpy(), oracle.magnification(full["count"], h.geometry.n_avg)))
+        band = sharded.row_bands(h.geometry.n2, world)[rank]
+        q.put((rank, ok, ok_mag, [st[k] for k in ("rays_in_map", "rays_outside", "rays_lost", "rays_total")],
+               [full["stats"][k] for k in ("rays_in_map", "rays_outside", "rays_lost", "rays_total")],
+               st["max_count"] == int(full["count"].max()), st["band"] == band,
+               h.calls == ["reset", ("band", 0, band[0], h.geometry.n1, band[1]), "mag"]))
     finally:
         dist.destroy_process_group()
 
 
-def test_two_rank_gloo_band_sum_equals_the_full_map():
+def test_two_rank_gloo_shoot_sharded_equals_the_full_map():
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
     procs = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
     for p in procs:
         p.start()
-    same, counters, full_counters, rays = q.get(timeout=180)
+    got = sorted(q.get(timeout=180) for _ in range(2))
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert same and counters == full_counters and counters[3] == rays
+    assert [g[0] for g in got] == [0, 1]
+    for rank, ok, ok_mag, counters, full_counters, ok_max, ok_band, ok_calls in got:  # identical result on every rank
+        assert ok and ok_mag and counters == full_counters and ok_max and ok_band and ok_calls, (rank, counters, full_counters)
 
 
 @pytest.mark.gpu
