@@ -18,6 +18,7 @@
 #include "mapstats_kernel.cuh"
 #include "shoot_kernel.cuh"
 #ifdef MLENS_ABLATIONS
+#include "shoot_ablation_kernels.cuh"
 #include "shoot_umma_kernel.cuh"
 #endif
 
@@ -43,6 +44,16 @@ int fail(int code, const char* fmt, ...) {
 
 constexpr int kChunkMax = 2048;        // lenses per chunk when the list is streamed in several chunks
 constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chunk
+// The production instantiation of shoot_fp32_kernel (chosen by the sweep in profiles/): tile width,
+// ray pairs per lens that share a reciprocal, resident CTAs per SM.
+#ifndef MLENS_PROD_TILE_X
+#define MLENS_PROD_TILE_X 64
+#endif
+#ifndef MLENS_PROD_SHARED_PAIRS
+#define MLENS_PROD_SHARED_PAIRS 0
+#endif
+constexpr int kProdTileX = MLENS_PROD_TILE_X, kProdSharedPairs = MLENS_PROD_SHARED_PAIRS;
+constexpr int kProdCtas = kProdTileX == 32 ? 3 : 2;
 constexpr int kTileCtrSlots = 256;     // ring of dynamic tile counters: one per launch in flight (see launch_block)
 
 }  // namespace
@@ -82,7 +93,8 @@ struct mlens {
     cudaEvent_t ev0, ev1, evk0, evk1;
     float last_ms, last_kernel_ms;
     // options
-    int opt_kernel, opt_binning, opt_ctas_per_sm, opt_shared, opt_rays;
+    int opt_kernel, opt_binning, opt_ctas_per_sm, opt_shared, opt_rays, opt_tile_x, opt_shared_pairs;
+    double lens_extent;                // max |coordinate| over the lens list (guards the shared-reciprocal products)
 };
 
 namespace {
@@ -107,7 +119,9 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     P.half_n1 = (double)h->geo.n1 / 2.0;
     P.half_n2 = (double)h->geo.n2 / 2.0;
     P.d = h->d;
-    P.tiles_x = (int)((ni + mlk::kTile - 1) / mlk::kTile);
+    // tile width: the production kernel's is an option; every other kernel walks 64 x 64 tiles
+    const int tile_x = h->opt_kernel == 1 ? h->opt_tile_x : mlk::kTile;
+    P.tiles_x = (int)((ni + tile_x - 1) / tile_x);
     P.tiles_y = (int)((nj + mlk::kTile - 1) / mlk::kTile);
     P.f1 = 1.0 - h->geo.kappa_s - h->gamma;
     P.f2 = 1.0 - h->geo.kappa_s + h->gamma;
@@ -119,7 +133,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     P.n_lens = (int)h->n_lens;
     P.rho2 = 0.25;  // rho = 0.5 sqrt(max(m,1))
     {
-        const double hd = 0.5 * mlk::kTile * h->d * 1.4142135623730951;  // tile half-diagonal
+        const double hd = 0.5 * h->d * std::sqrt((double)tile_x * tile_x + (double)mlk::kTile * mlk::kTile);  // tile half-diagonal
         P.rho2_tile = 4.0 * hd * hd;
     }
     P.count = count; P.ray_y = ray_y; P.ray_pix = ray_pix;
@@ -196,23 +210,51 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     P.chunk = chunk; P.n_chunks = n_chunks;
     const size_t smem = sizeof(mlk::TileShared) + (size_t)chunk * 16 * (n_chunks > 1 ? 3 : 2);
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
-    long long grid = (long long)h->sm_count * h->opt_ctas_per_sm;
-    if (grid > n_tiles) grid = n_tiles;
     void (*kern)(const mlk::ShootParams) = nullptr;
-    const int code = h->opt_rays * 100 + h->opt_shared;
-    switch (code) {
-#define MLENS_VARIANT(R, SH) case R * 100 + SH: kern = mlk::shoot_fp32_kernel<R, SH, -1>; break;
-        MLENS_VARIANT(8, 0)
+    int threads = 0, ctas = 0;
+
 #ifdef MLENS_ABLATIONS
-        MLENS_VARIANT(16, 0) MLENS_VARIANT(16, 1) MLENS_VARIANT(16, 2) MLENS_VARIANT(16, 3) MLENS_VARIANT(16, 4)
-        MLENS_VARIANT(8, 1) MLENS_VARIANT(8, 2)
+    if (h->opt_kernel == 4) {  // the round-1 production kernel (A/B baseline) and its shared-reciprocal variants
+        switch (h->opt_shared) {
+            case 0: kern = mlk::shoot_fp32_r1_kernel<8, 0, -1>; break;
+            case 1: kern = mlk::shoot_fp32_r1_kernel<8, 1, -1>; break;
+            case 2: kern = mlk::shoot_fp32_r1_kernel<8, 2, -1>; break;
+            default: return fail(MLENS_EINVAL, "kernel 4 has shared_rcp 0..2");
+        }
+        threads = 512; ctas = 2;
+    }
+#endif
+    if (!kern) {
+        // Shared reciprocals multiply two squared distances in lattice units: keep the product inside FP32 (the lattice
+        // has < 2^31 rays per axis, but the caller's lenses may lie anywhere).  Beyond that, one MUFU.RCP per ray.
+        int shared = h->opt_shared_pairs;
+        const double zmax = (h->lens_extent + std::fmax(h->geo.a1, h->geo.a2)) / h->d;  // per axis, lattice units
+        if (shared > 0 && 4.0 * zmax * zmax * zmax * zmax > 1.0e37) shared = 0;
+        const int code = h->opt_tile_x * 10 + shared;
+        const bool runs = h->opt_binning == mlk::BIN_RUNS;  // the default binning route is compiled in (shorter epilogue)
+        switch (code) {
+#define MLENS_VARIANT(TX, SP, NC)                                                                        \
+    case TX * 10 + SP:                                                                                   \
+        kern = runs ? mlk::shoot_fp32_kernel<TX, 8, SP, NC, mlk::BIN_RUNS> : mlk::shoot_fp32_kernel<TX, 8, SP, NC, -1>; \
+        threads = TX / 8 * mlk::kTile; ctas = NC;                                                        \
+        break;
+#ifdef MLENS_ABLATIONS  // the whole sweep grid: tile width x shared pairs
+#define MLENS_SWEEP(SP) MLENS_VARIANT(64, SP, 2) MLENS_VARIANT(48, SP, 2) MLENS_VARIANT(32, SP, 3)
+            MLENS_SWEEP(0) MLENS_SWEEP(1) MLENS_SWEEP(2) MLENS_VARIANT(64, 3, 2) MLENS_VARIANT(64, 4, 2)
+#undef MLENS_SWEEP
+#else                   // the shipped library: the production instantiation and its one-reciprocal-per-ray fallback
+            MLENS_VARIANT(kProdTileX, 0, kProdCtas)
+#if MLENS_PROD_SHARED_PAIRS != 0
+            MLENS_VARIANT(kProdTileX, kProdSharedPairs, kProdCtas)
+#endif
 #endif
 #undef MLENS_VARIANT
-        default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d shared_rcp=%d", h->opt_rays, h->opt_shared);
+            default: return fail(MLENS_EINVAL, "no kernel variant tile_x=%d shared_pairs=%d in this build", h->opt_tile_x, shared);
+        }
     }
-    // the production configuration has its binning route compiled in (shorter epilogue)
-    if (code == 800 && h->opt_binning == mlk::BIN_RUNS) kern = mlk::shoot_fp32_kernel<8, 0, mlk::BIN_RUNS>;
-    const int threads = mlk::kTile * mlk::kTile / h->opt_rays;
+    if (h->opt_ctas_per_sm > 0) ctas = h->opt_ctas_per_sm;
+    long long grid = (long long)h->sm_count * ctas;
+    if (grid > n_tiles) grid = n_tiles;
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<(unsigned)grid, threads, smem, st>>>(P);
     MLENS_CUDA(cudaGetLastError());
@@ -309,7 +351,10 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
     h->npix = npix; h->n_lens = n_lens; h->geo = g;
     h->device = dev; h->sm_count = prop.multiProcessorCount;
-    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 2; h->opt_shared = 0; h->opt_rays = 8;
+    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 0; h->opt_shared = 0; h->opt_rays = 8;
+    h->opt_tile_x = kProdTileX; h->opt_shared_pairs = kProdSharedPairs;
+    for (long long k = 0; k < n_lens; ++k)
+        h->lens_extent = std::fmax(h->lens_extent, std::fmax(std::fabs((double)packed[(size_t)k].x), std::fabs((double)packed[(size_t)k].y)));
 
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
@@ -374,24 +419,28 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
     // the shipped library holds the production kernel only: the debug / ablation / experimental kernels and loop variants
     // exist in the MLENS_ABLATIONS build (libmlens_ablations.so, used by the tests and the profiling runs)
     if ((!strcmp(key, "kernel") && value != 1) || (!strcmp(key, "shared_rcp") && value != 0) ||
-        (!strcmp(key, "rays_per_thread") && value != 8))
+        (!strcmp(key, "tile_x") && value != kProdTileX) ||
+        (!strcmp(key, "shared_pairs") && value != 0 && value != kProdSharedPairs))
         return fail(MLENS_EINVAL, "option %s=%lld needs the MLENS_ABLATIONS build of the library", key, value);
 #endif
     if (!strcmp(key, "kernel")) {
-        if (value < 0 || value > 3) return fail(MLENS_EINVAL, "kernel must be 0..3");
+        if (value < 0 || value > 4) return fail(MLENS_EINVAL, "kernel must be 0..4");
         h->opt_kernel = (int)value;
+    } else if (!strcmp(key, "tile_x")) {
+        if (value != 64 && value != 48 && value != 32) return fail(MLENS_EINVAL, "tile_x must be 64, 48 or 32");
+        h->opt_tile_x = (int)value;
+    } else if (!strcmp(key, "shared_pairs")) {
+        if (value < 0 || value > 4) return fail(MLENS_EINVAL, "shared_pairs must be 0..4");
+        h->opt_shared_pairs = (int)value;
     } else if (!strcmp(key, "binning")) {
         if (value < 0 || value > 3) return fail(MLENS_EINVAL, "binning must be 0..3");
         h->opt_binning = (int)value;
     } else if (!strcmp(key, "ctas_per_sm")) {
-        if (value < 1 || value > 8) return fail(MLENS_EINVAL, "ctas_per_sm must be 1..8");
+        if (value < 0 || value > 8) return fail(MLENS_EINVAL, "ctas_per_sm must be 0 (the kernel's own) or 1..8");
         h->opt_ctas_per_sm = (int)value;
     } else if (!strcmp(key, "shared_rcp")) {
-        if (value < 0 || value > 4) return fail(MLENS_EINVAL, "shared_rcp must be 0..4");
+        if (value < 0 || value > 2) return fail(MLENS_EINVAL, "shared_rcp must be 0..2");
         h->opt_shared = (int)value;
-    } else if (!strcmp(key, "rays_per_thread")) {
-        if (value != 8 && value != 16) return fail(MLENS_EINVAL, "rays_per_thread must be 8 or 16");
-        h->opt_rays = (int)value;
     } else {
         return fail(MLENS_EINVAL, "unknown option '%s'", key);
     }

@@ -1,6 +1,6 @@
 // shoot_kernel.cuh — sm_100a device code of libmlens.so.
 //
-// shoot_fp32_kernel: the production kernel.  Persistent CTAs walk 64x64-ray tiles of the image-plane lattice
+// shoot_fp32_kernel: the production kernel.  Persistent CTAs walk kTX x 64-ray tiles of the image-plane lattice
 // (Fig. 1).  For every ray the deflection of Eq. (1) is summed DIRECTLY over all N_*
 // lenses, in the algebraically identical "difference form" that keeps FP32 rounding harmless:
 //
@@ -10,10 +10,18 @@
 //   =>  conj(alpha) = A_c - delta * S(delta),   A_c = sum_i c_i (FP64, once per tile),
 //                                               S   = sum_i c_i conj(w_i)/|w_i|^2,  w_i = zeta_i + delta  (FP32 loop)
 //
-// Per interaction: 1 packed FADD2 + 5 packed FFMA2 per PAIR of rays and one MUFU.RCP per ray.  Lenses within rho of
-// the tile centre are summed per ray in plain FP64 instead (near list).  The per-ray epilogue (Eq. 1 macro term,
-// pixel id) is FP64; binning ("accumulated on a gridded source plane") uses integer REDs, so the map does
-// not depend on the order of execution.
+// The FP32 loop works in LATTICE UNITS (lengths / d: in-tile offsets are exact half-integers) and around the THREAD
+// centre: a thread owns kR consecutive rays of one row at offsets eps = +-1/2, +-3/2, ... from its centre w_t, and
+//       c conj(w_t + eps) = c conj(w_t) + eps c            (eps real)
+//   =>  S(eps) = A' + eps P + i (B' + eps Q),   A' + i B' = sum_i rc_i c_i conj(w_t,i),   P + i Q = sum_i rc_i c_i,
+//       rc_i = 1/|w_t,i + eps|^2,   |w_t + eps|^2 = (|w_t|^2 + eps^2) +- 2 |eps| Re(w_t)
+// so that per lens a thread does ~8 scalar FP32 operations for the terms shared by its rays, and per ray 1.5 FMA-pipe
+// operations for r^2 (literal constants), ONE MUFU.RCP (or half of one: kSharedPairs) and four accumulations whose
+// multiplier is a lens-uniform scalar — packed FFMA2 with only two register-pair operands, which run at the full
+// 2 clk/warp (the round-1 form's two accumulations per pair read three register pairs: 3.1 clk).
+// Lenses within rho of the tile centre are summed per ray in plain FP64 instead (near list).  The per-ray epilogue
+// (Eq. 1 macro term, pixel id) is FP64; binning ("accumulated on a gridded source plane") uses integer
+// REDs, so the map does not depend on the order of execution.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -25,8 +33,8 @@
 namespace mlk {
 
 constexpr int kHotUnroll = MLENS_HOT_UNROLL;
-constexpr int kTile = 64;           // tile is kTile x kTile rays
-constexpr int kMaxThreads = 512;    // threads per CTA = kTile*kTile/kR (kR rays per thread, consecutive along x1)
+constexpr int kTile = 64;           // tile height in rays (rows); also the width of the round-1 / ablation kernels' tiles
+constexpr int kMaxThreads = 512;    // most threads per CTA of any variant (tile width / rays per thread x 64 rows)
 constexpr int kNearMax = 32;        // capacity of the per-tile near-lens list
 constexpr int kWin = 32;            // binning window side (pixels), BIN_WINDOW mode
 constexpr float kFar = 1.0e8f;      // offset of a neutralised main-list entry (c = 0: contributes exactly 0;
@@ -39,7 +47,7 @@ struct ShootParams {
     long long i0, j0, ni, nj;       // block of rays to shoot
     double half_n1, half_n2;        // n1/2, n2/2
     double d;                       // ray spacing
-    int tiles_x, tiles_y;
+    int tiles_x, tiles_y;           // tiles of the block: ceil(ni / tile width) x ceil(nj / 64)
     // macro model and map
     double f1, f2;                  // 1-kappa_s-gamma, 1-kappa_s+gamma
     double half_L, p, inv_p;        // L/2, pixel size and 1/p
@@ -93,6 +101,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
 }
 __device__ __forceinline__ float rcp_mufu(float x) {
+#ifdef MLENS_PROBE_NO_MUFU  // profiling builds only (profiles/): a crude integer-pipe stand-in, to time the FMA side alone
+    return __int_as_float(0x7EF311C7 - __float_as_int(x));
+#endif
     float r;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
     return r;
@@ -135,6 +146,8 @@ struct __align__(16) TileShared {
     uint64_t bar[2];                         // mbarriers of the raw-chunk double buffer
     double part[kMaxThreads / 32][2];        // per-warp partial sums of A_c
     double near_zx[kNearMax], near_zy[kNearMax], near_m[kNearMax];
+    double sort_zx[kNearMax], sort_zy[kNearMax], sort_m[kNearMax];  // the near list in lens order (canonical summation order)
+    int near_idx[kNearMax];
     int near_n;
     int win_ix0, win_iy0;                    // binning window origin (BIN_WINDOW)
     long long next_tile;                     // the CTA's next tile, fetched from the global counter by thread 0
@@ -159,18 +172,104 @@ __device__ __forceinline__ void flush_run(const ShootParams& P, TileShared& sh, 
     }
 }
 
-// kShared = number of the thread's 4-ray groups (two packed ray pairs A, B) per lens whose four reciprocals come from
-// TWO MUFU.RCP instead of four, with packed multiplies only:
-//   q = r2A * r2B (FMUL2);  t = (rcp q.x, rcp q.y);  1/r2A = t * r2B (FMUL2);  1/r2B = t * r2A (FMUL2)
-// Kept as an ablation switch only: measured on B200 it LOSES (150.7 -> 159.2 -> 175.8 ms for 0/1/2 shared groups,
-// profiles/r1_summary.md).  Packed FP32 instructions with three distinct register-pair operands are bound by
-// register-file read bandwidth (3.0 clk, not 2.0), so the three extra FMUL2 cost more than the two MUFU they save.
-// kBin >= 0 fixes the binning route at compile time (the production instantiation: BIN_RUNS); kBin < 0 reads P.bin_mode.
-template <int kR, int kShared, int kBin>
-__global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const ShootParams P) {
+
+// The rare per-ray path of the epilogue: tiles with a near-lens list (those lenses are summed here in plain FP64, in lens
+// order) or with a list overflow (the ray takes Eq. (1) over ALL lenses in plain FP64 from global memory).  Kept out of
+// line so that its loops and FP64 temporaries do not inflate the register budget of the common path.
+//   al1, al2 in: deflection of the FP32 list (A_c - delta*S); dxd, dyt: exact FP64 in-tile offsets; x1, x2: ray position
+__device__ __noinline__ double2 special_ray(const ShootParams& P, const TileShared& sh, int n_near, bool near_overflow,
+                                            double al1, double al2, double dxd, double dyt, double x1, double x2) {
+    for (int q = 0; q < n_near; ++q) {
+        const double wx = sh.sort_zx[q] + dxd, wy = sh.sort_zy[q] + dyt;
+        const double f = sh.sort_m[q] / (wx * wx + wy * wy);
+        al1 += f * wx;
+        al2 += f * wy;
+    }
+    if (near_overflow) {
+        // more than kNearMax lenses within rho of this tile: the FP32 list then holds lenses it cannot sum accurately
+        // (or at all: r2 = 0), so the tile's rays take Eq. (1) in plain FP64 from global memory
+        al1 = al2 = 0.0;
+        for (int q = 0; q < P.n_lens; ++q) {
+            const float4 l = __ldg(P.lens_raw + q);
+            const double wx = x1 - (double)l.x, wy = x2 - (double)l.y;
+            const double f = (double)l.z / (wx * wx + wy * wy);
+            al1 += f * wx;
+            al2 += f * wy;
+        }
+    }
+    return make_double2((P.f1 * x1 - al1 + P.half_L) * P.inv_p, (P.f2 * x2 - al2 + P.half_L) * P.inv_p);
+}
+
+// Which ray of a thread sits in which lane of which accumulator pair.  Ray k (k = 0..kR-1, left to right) is at
+// eps = k - (kR-1)/2 lattice steps from the thread centre.  Pairs hold two rays on the SAME side of the centre:
+// pairs 0..kR/4-1 the rays at eps = +(2j + 1/2), +(2j + 3/2); pairs kR/4.. the mirror images (eps < 0) in the same order,
+// so that r^2 of a pair and of its mirror pair share the packed constants (2|eps|) and the packed (|w_t|^2 + eps^2).
+template <int kR>
+struct RayMap {
+    static_assert(kR % 4 == 0, "rays per thread: a multiple of 4");
+    __host__ __device__ static constexpr int pair_of(int k) { return k >= kR / 2 ? (k - kR / 2) / 2 : kR / 4 + (kR / 2 - 1 - k) / 2; }
+    __host__ __device__ static constexpr bool hi_of(int k) { return k >= kR / 2 ? ((k - kR / 2) & 1) : ((kR / 2 - 1 - k) & 1); }
+};
+
+// One lens x the kR rays of a thread.  q = (Re w', Im w', c'_r, c'_i) of the lens relative to the TILE centre in
+// lattice units; cxf / dyf = the thread centre's in-tile offset.  (A', B', P, Q)[j] = the four sums of ray pair j.
+template <int kR, int kSharedPairs>
+__device__ __forceinline__ void interact(const float4 q, const float cxf, const float dyf, float2 (&A)[kR / 2],
+                                         float2 (&B)[kR / 2], float2 (&Pp)[kR / 2], float2 (&Qq)[kR / 2]) {
+    const float ux = q.x + cxf;                        // Re(w_t)
+    const float wy = q.y + dyf;                        // Im(w_t)
+    const float G0 = fmaf(ux, ux, wy * wy);            // |w_t|^2
+    const float ap = fmaf(q.z, ux, q.w * wy);          // Re(c conj(w_t))
+    const float bp = fmaf(q.w, ux, -(q.z * wy));       // Im(c conj(w_t))
+    const float2 UX = make_float2(ux, ux), NUX = make_float2(-ux, -ux), GG = make_float2(G0, G0);
+    float2 r2[kR / 2], rc[kR / 2];
+    // |w_t + eps|^2 = (|w_t|^2 + eps^2) + 2 eps Re(w_t): packed, the constants are literals
+#pragma unroll
+    for (int j = 0; j < kR / 4; ++j) {
+        const float e0 = 2.0f * (float)j + 0.5f, e1 = e0 + 1.0f;
+        const float2 Gj = __fadd2_rn(GG, make_float2(e0 * e0, e1 * e1));
+        const float2 Ej = make_float2(2.0f * e0, 2.0f * e1);
+        r2[j] = __ffma2_rn(Ej, UX, Gj);
+        r2[kR / 4 + j] = __ffma2_rn(Ej, NUX, Gj);
+    }
+    // reciprocals: the first kSharedPairs pairs take 1/r2 of two rays from ONE MUFU.RCP of the product of the two r2
+    // (3 FMUL + 1 MUFU per two rays instead of 2 MUFU): worth it only while the FMA pipe has the slack
+#pragma unroll
+    for (int j = 0; j < kR / 2; ++j) {
+        if (j + 1 < kSharedPairs) {                    // two pairs at once, packed: 3 FMUL2 + 2 MUFU for four rays
+            if ((j & 1) == 0) {
+                const float2 qq = __fmul2_rn(r2[j], r2[j + 1]);
+                const float2 t = make_float2(rcp_mufu(qq.x), rcp_mufu(qq.y));
+                rc[j] = __fmul2_rn(t, r2[j + 1]);
+                rc[j + 1] = __fmul2_rn(t, r2[j]);
+            }
+        } else if (j < kSharedPairs && (j & 1) == 0) { // a single left-over pair: the two rays of the pair share
+            const float t = rcp_mufu(r2[j].x * r2[j].y);
+            rc[j] = make_float2(t * r2[j].y, t * r2[j].x);
+        } else if (j >= kSharedPairs) {
+            rc[j] = make_float2(rcp_mufu(r2[j].x), rcp_mufu(r2[j].y));
+        }
+    }
+    const float2 AP = make_float2(ap, ap), BP = make_float2(bp, bp), CR = make_float2(q.z, q.z), CI = make_float2(q.w, q.w);
+#pragma unroll
+    for (int j = 0; j < kR / 2; ++j) {
+        A[j] = __ffma2_rn(AP, rc[j], A[j]);
+        B[j] = __ffma2_rn(BP, rc[j], B[j]);
+        Pp[j] = __ffma2_rn(CR, rc[j], Pp[j]);
+        Qq[j] = __ffma2_rn(CI, rc[j], Qq[j]);
+    }
+}
+
+// kTX = tile width in rays (the tile is kTX x 64), kR = rays per thread (consecutive along x1), kSharedPairs = ray pairs
+// per lens whose two reciprocals come from one MUFU.RCP, kMinCtas = resident CTAs per SM the register budget is cut for,
+// kBin >= 0 fixes the binning route at compile time (production: BIN_RUNS); kBin < 0 reads P.bin_mode.
+template <int kTX, int kR, int kSharedPairs, int kMinCtas, int kBin>
+__global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(const __grid_constant__ ShootParams P) {
+    static_assert(kR % 2 == 0 && kTX % kR == 0 && kTX % 2 == 0, "tile width: a whole number of threads, even");
     const int bin_mode = kBin >= 0 ? kBin : P.bin_mode;
-    constexpr int kThreads = kTile * kTile / kR;
-    constexpr int kTx = kTile / kR;  // threads along x1
+    constexpr int kThreads = kTX / kR * kTile;
+    constexpr int kTx = kTX / kR;  // threads along x1
+    static_assert(kThreads <= kMaxThreads && kThreads % 32 == 0, "CTA size");
     extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
     TileShared& sh = *reinterpret_cast<TileShared*>(smem_raw_bytes);
     float4* xf = reinterpret_cast<float4*>(smem_raw_bytes + sizeof(TileShared));  // transformed chunk
@@ -189,16 +288,11 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
     }
     __syncthreads();
 
-    // in-tile offsets delta (FP32), identical for every tile
-    const float dyf = (float)(((double)ty - 31.5) * P.d);
-    float2 dxb[kR / 2];
-#pragma unroll
-    for (int j = 0; j < kR / 2; ++j) {
-        dxb[j].x = (float)(((double)(tx * kR + 2 * j) - 31.5) * P.d);
-        dxb[j].y = (float)(((double)(tx * kR + 2 * j + 1) - 31.5) * P.d);
-    }
+    // in-tile offsets of the thread centre from the tile centre, in lattice steps: exact small (half-)integers
+    const float cxf = (float)(tx * kR + kR / 2 - kTX / 2);
+    const float dyf = (float)ty - 31.5f;
+    const double inv_d = 1.0 / P.d;
 
-    const double dxt0 = (double)(tx * kR) - 31.5;  // in-tile offset of the thread's first ray, in lattice steps
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
     long long g = 0;  // sequence number of the raw-chunk load being consumed: buffer g&1, barrier phase (g>>1)&1
 
@@ -209,23 +303,23 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
         bulk_copy_g2s(raw0, P.lens_raw, bytes, &sh.bar[0]);
     }
 
-    // DYNAMIC tile scheduling.  Tiles are equal work, but the warp scheduler favours the older of an SM's two CTAs: with a
-    // static split the older one finished its share after ~65 % of the kernel and the other ran the rest alone, with its
-    // per-tile bookkeeping exposed (alone: 84 % of the paired rate at N* = 430, 92 % at N* = 2333).  Every CTA takes its
-    // first tile by index and every further one from a global counter, fetched one tile ahead by thread 0 so that the
-    // atomic's latency is hidden; all CTAs now finish within one tile of each other.  (Which CTA shoots a tile does not
-    // affect its arithmetic, and the map is built from integer REDs, so the result is unchanged.)
+    // DYNAMIC tile scheduling.  Tiles are equal work, but the warp scheduler favours the older of an SM's CTAs: with a
+    // static split the older one finished its share after ~65 % of the kernel and the others ran the rest alone, with
+    // their per-tile bookkeeping exposed.  Every CTA takes its first tile by index and every further one from a global
+    // counter (one per launch), fetched one tile ahead by thread 0 so that the atomic's latency is hidden; all CTAs
+    // finish within one tile of each other.  (Which CTA shoots a tile does not affect its arithmetic, and the map is
+    // built from integer REDs, so the result is unchanged.)
     long long nxt = 0;  // thread 0 only
     for (long long tile = blockIdx.x; tile < n_tiles;) {
         if (tid == 0) nxt = (long long)atomicAdd(P.tile_counter, 1ull) + gridDim.x;
         const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
-        const long long ti0 = P.i0 + (long long)tI * kTile, tj0 = P.j0 + (long long)tJ * kTile;
-        const double Zcx = ((double)(ti0 + kTile / 2) - P.half_n1) * P.d;
+        const long long ti0 = P.i0 + (long long)tI * kTX, tj0 = P.j0 + (long long)tJ * kTile;
+        const double Zcx = ((double)(ti0 + kTX / 2) - P.half_n1) * P.d;
         const double Zcy = ((double)(tj0 + kTile / 2) - P.half_n2) * P.d;
 
-        float2 Sr[kR / 2], Si[kR / 2];
+        float2 A[kR / 2], B[kR / 2], Pp[kR / 2], Qq[kR / 2];
 #pragma unroll
-        for (int j = 0; j < kR / 2; ++j) Sr[j] = Si[j] = make_float2(0.f, 0.f);
+        for (int j = 0; j < kR / 2; ++j) A[j] = B[j] = Pp[j] = Qq[j] = make_float2(0.f, 0.f);
         double Acr = 0.0, Aci = 0.0;
 
         for (int c = 0; c < P.n_chunks && P.n_lens > 0; ++c) {
@@ -235,7 +329,8 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
             float4* raw = raw0 + (size_t)buf * P.chunk;
             // (1) raw chunk landed?  (single-chunk lists are staged once and stay resident: only load 0 is waited for)
             if (P.n_chunks > 1 || tile == (long long)blockIdx.x) mbar_wait(&sh.bar[buf], (uint32_t)((g >> 1) & 1));
-            // (2) per-tile FP64 transform: zeta = Z_c - z_i, c = m/zeta; near lenses go to the FP64 list
+            // (2) per-tile FP64 transform: zeta = Z_c - z_i, c = m/zeta, both divided by d (lattice units) and rounded
+            //     to FP32; near lenses go to the FP64 list
             double pr_ = 0.0, pi_ = 0.0;
             const int n_pad = (n_c + 3) & ~3;
             for (int t = tid; t < n_pad; t += kThreads) {
@@ -248,16 +343,16 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
                     if (near) {
                         const int slot = atomicAdd(&sh.near_n, 1);
                         if (slot < kNearMax) {
-                            sh.near_zx[slot] = zx; sh.near_zy[slot] = zy; sh.near_m[slot] = m;
+                            sh.near_zx[slot] = zx; sh.near_zy[slot] = zy; sh.near_m[slot] = m; sh.near_idx[slot] = l0 + t;
                         } else {
-                            near = false;  // list full: keep the lens in the FP32 list (still summed, less accurate)
+                            near = false;  // list full: keep the lens in the FP32 list (the tile takes the FP64 fallback)
                         }
                     }
                     if (!near) {
                         const double inv = m / r2;
                         const double cr = zx * inv, ci = -zy * inv;
                         pr_ += cr; pi_ += ci;
-                        o = make_float4((float)zx, (float)zy, (float)cr, (float)ci);
+                        o = make_float4((float)(zx * inv_d), (float)(zy * inv_d), (float)(cr * inv_d), (float)(ci * inv_d));
                     }
                 }
                 xf[t] = o;
@@ -289,47 +384,43 @@ __global__ void __launch_bounds__(kTile * kTile / kR, 2) shoot_fp32_kernel(const
             float4 qn = xf[0];
 #pragma unroll kHotUnroll
             for (int l = 0; l < n_pad; ++l) {
-                const float4 q = qn;  // (zeta_x, zeta_y, c_r, c_i)
+                const float4 q = qn;  // (zeta_x, zeta_y, c_r, c_i) / d
                 qn = xf[l + 1];       // broadcast LDS.128 one lens ahead (xf[n_pad] is readable: raw0 follows xf)
-                const float dy = dyf + q.y;
-                const float dy2 = dy * dy;
-                const float a = q.w * dy;    //  c_i * dy
-                const float b = -q.z * dy;   // -c_r * dy
-                const float2 NX = make_float2(q.x, q.x), DY2 = make_float2(dy2, dy2);
-                const float2 AA = make_float2(a, a), BB = make_float2(b, b);
-                const float2 CR = make_float2(q.z, q.z), CI = make_float2(q.w, q.w);
-float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
-#pragma unroll
-                for (int j = 0; j < kR / 2; ++j) {
-                    dx[j] = __fadd2_rn(dxb[j], NX);
-                    r2[j] = __ffma2_rn(dx[j], dx[j], DY2);
-                }
-#pragma unroll
-                for (int j = 0; j < kR / 2; j += 2) {
-                    if (j / 2 < kShared) {
-                        const float2 qq = __fmul2_rn(r2[j], r2[j + 1]);
-                        const float2 t = make_float2(rcp_mufu(qq.x), rcp_mufu(qq.y));
-                        rc[j] = __fmul2_rn(t, r2[j + 1]);
-                        rc[j + 1] = __fmul2_rn(t, r2[j]);
-                    } else {
-                        rc[j] = make_float2(rcp_mufu(r2[j].x), rcp_mufu(r2[j].y));
-                        rc[j + 1] = make_float2(rcp_mufu(r2[j + 1].x), rcp_mufu(r2[j + 1].y));
-                    }
-                }
-#pragma unroll
-                for (int j = 0; j < kR / 2; ++j) {
-                    const float2 pr = __ffma2_rn(CR, dx[j], AA);
-                    const float2 pi = __ffma2_rn(CI, dx[j], BB);
-                    Sr[j] = __ffma2_rn(pr, rc[j], Sr[j]);
-                    Si[j] = __ffma2_rn(pi, rc[j], Si[j]);
-                }
+                interact<kR, kSharedPairs>(q, cxf, dyf, A, B, Pp, Qq);
             }
             __syncthreads();  // xf (and sh.part) may be overwritten by the next chunk / tile
         }
 
         // (5) per-ray FP64 epilogue: alpha, Eq. (1), pixel id; (6) binning
-        const int n_near = min(sh.near_n, kNearMax);
+        // first the four sums of every ray collapse to S = A' + eps P + i (B' + eps Q): 2 kR live values instead of 4 kR.
+        // ray k of the thread sits at eps = k - (kR-1)/2 from the thread centre (pair and lane: RayMap)
+        float sre[kR], sim[kR];
+#pragma unroll
+        for (int k = 0; k < kR; ++k) {
+            constexpr int kDummy = 0; (void)kDummy;
+            const int j = RayMap<kR>::pair_of(k);
+            const bool hi = RayMap<kR>::hi_of(k);
+            const float eps = (float)k - 0.5f * (float)(kR - 1);
+            sre[k] = fmaf(eps, hi ? Pp[j].y : Pp[j].x, hi ? A[j].y : A[j].x);
+            sim[k] = fmaf(eps, hi ? Qq[j].y : Qq[j].x, hi ? B[j].y : B[j].x);
+        }
+        int n_near = min(sh.near_n, kNearMax);
         const bool near_overflow = sh.near_n > kNearMax;
+        if (n_near > 1 && !near_overflow) {
+            // canonical summation order: the slots were handed out by an atomic, i.e. in an order that varies from run
+            // to run; the per-ray FP64 sums below run over the list sorted by lens index, so the map is reproducible
+            if (tid < n_near) {
+                const int me = sh.near_idx[tid];
+                int rank = 0;
+                for (int q = 0; q < n_near; ++q) rank += (sh.near_idx[q] < me);
+                sh.sort_zx[rank] = sh.near_zx[tid]; sh.sort_zy[rank] = sh.near_zy[tid]; sh.sort_m[rank] = sh.near_m[tid];
+            }
+            __syncthreads();
+        } else if (n_near == 1) {
+            if (tid == 0) { sh.sort_zx[0] = sh.near_zx[0]; sh.sort_zy[0] = sh.near_zy[0]; sh.sort_m[0] = sh.near_m[0]; }
+            __syncthreads();
+        }
+        if (near_overflow) n_near = 0;  // the FP64 fallback sums ALL lenses from global memory, in input order
         const long long jray = tj0 + ty;
         const bool row_ok = jray < P.j0 + P.nj;
         const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
@@ -350,63 +441,41 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
 
         // Source position in PIXEL units, u = (y + L/2)/p.  Everything large is folded into one FP64 constant per tile,
         //   U_c = (f * Z_c -+ A_c + L/2) / p,
-        // and a ray adds only its small in-tile part: u = U_c + (f*delta_true -+ delta*S)/p, where delta*S is formed in
-        // FP32 (its own rounding, ~1e-9 R_E, is below that of the S accumulators) and delta_true is the exact FP64
-        // in-tile offset.  One multiply by 1/p replaces the divide; against the oracle's (y + L/2)/p this moves u by
-        // a few ulp (1e-13 px), far inside the 1e-3 px exemption band of the parity tolerance.
+        // and a ray adds only its small in-tile part: u = U_c + (f*delta -+ delta*S)/p, where delta*S is formed in
+        // FP32 in lattice units (its own rounding is below that of the accumulators) and delta is the exact in-tile
+        // offset.  One multiply by 1/p replaces the divide; against the oracle's (y + L/2)/p this moves u by a few ulp
+        // (1e-13 px), far inside the 1e-3 px exemption band of the parity tolerance.
         const double U1c = (P.f1 * Zcx - Acr + P.half_L) * P.inv_p;
         const double U2c = (P.f2 * Zcy + Aci + P.half_L) * P.inv_p;
-        const double dyt = ((double)ty - 31.5) * P.d;
-        const double row2 = P.f2 * dyt;
-        const bool special = n_near > 0 || near_overflow;  // tile-uniform: near-lens list or FP64 fallback in play
+        const double dyt = ((double)ty - 31.5) * P.d;        // exact in-tile offsets in R_E
+        const bool special = n_near > 0 || near_overflow;    // tile-uniform: near-lens list or FP64 fallback in play
         const bool want_rays = P.ray_y != nullptr || P.ray_pix != nullptr;
         const double npix_d = (double)P.npix;
-        // u1 of ray k = B1 + k*s1 + (delta*S)_re / p  with the thread's first in-tile offset folded into B1
-        const double s1 = P.f1 * P.d * P.inv_p;
+        const double dip = P.d * P.inv_p;                     // lattice step in pixels
+        // u1 of ray k = B1 + k*s1 + (delta*S)_re * d/p  with the thread's first in-tile offset folded into B1
+        const double s1 = P.f1 * dip;
+        const double dxt0 = (double)(tx * kR) + 0.5 - (double)(kTX / 2);  // first ray's in-tile offset, lattice steps
         const double B1 = fma(dxt0, s1, U1c);
-        const double B2 = fma(row2, P.inv_p, U2c);
+        const double B2 = fma(P.f2 * dyt, P.inv_p, U2c);
 
 #pragma unroll
         for (int k = 0; k < kR; ++k) {
-            const int j = k >> 1;
-            const float srf = (k & 1) ? Sr[j].y : Sr[j].x;
-            const float sif = (k & 1) ? Si[j].y : Si[j].x;
-            const float dxf = (k & 1) ? dxb[j].y : dxb[j].x;
+            const float eps = (float)k - 0.5f * (float)(kR - 1);
+            const float srf = sre[k], sif = sim[k];
+            const float dxf = cxf + eps;                     // in-tile offset in lattice steps (exact)
             const long long iray = ti0 + tx * kR + k;
             const bool ok = row_ok && iray < P.i0 + P.ni;
             // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im);  y1 = f1 x1 - alpha1,  y2 = f2 x2 - alpha2
-            const float ds_re = dxf * srf - dyf * sif;
+            const float ds_re = dxf * srf - dyf * sif;       // (delta * S) / d
             const float ds_im = dxf * sif + dyf * srf;
-            double u1 = fma(f32_to_f64_bits(ds_re), P.inv_p, fma((double)k, s1, B1));
-            double u2 = fma(-f32_to_f64_bits(ds_im), P.inv_p, B2);
+            double u1 = fma(f32_to_f64_bits(ds_re), dip, fma((double)k, s1, B1));
+            double u2 = fma(-f32_to_f64_bits(ds_im), dip, B2);
             bool finite = fabsf(ds_re) <= 3.4028234663852886e38f && fabsf(ds_im) <= 3.4028234663852886e38f;
             if (special) {
-                // exact FP64 in-tile offsets here: the float-rounded ones are off by ~1e-9 R_E, which a ray 1e-4 R_E from
-                // a lens (deflection gradient m/r^2 ~ 1e8) turns into tens of pixels
-                const double dxd = (dxt0 + (double)k) * P.d;
-                double al1 = Acr - (double)ds_re;
-                double al2 = -(Aci - (double)ds_im);
-                for (int q = 0; q < n_near; ++q) {
-                    const double wx = sh.near_zx[q] + dxd, wy = sh.near_zy[q] + dyt;
-                    const double f = sh.near_m[q] / (wx * wx + wy * wy);
-                    al1 += f * wx;
-                    al2 += f * wy;
-                }
-                const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
-                if (near_overflow) {
-                    // more than kNearMax lenses within rho of this tile: the FP32 list then holds lenses it cannot sum
-                    // accurately (or at all: r2 = 0), so the tile's rays take Eq. (1) in plain FP64 from global memory
-                    al1 = al2 = 0.0;
-                    for (int q = 0; q < P.n_lens; ++q) {
-                        const float4 l = __ldg(P.lens_raw + q);
-                        const double wx = x1 - (double)l.x, wy = x2 - (double)l.y;
-                        const double f = (double)l.z / (wx * wx + wy * wy);
-                        al1 += f * wx;
-                        al2 += f * wy;
-                    }
-                }
-                u1 = (P.f1 * x1 - al1 + P.half_L) * P.inv_p;
-                u2 = (P.f2 * x2 - al2 + P.half_L) * P.inv_p;
+                // exact FP64 in-tile offsets here: a ray 1e-4 R_E from a lens sees a deflection gradient m/r^2 ~ 1e8
+                const double2 u = special_ray(P, sh, n_near, near_overflow, Acr - (double)ds_re * P.d, -(Aci - (double)ds_im * P.d),
+                                              (dxt0 + (double)k) * P.d, dyt, ((double)iray + 0.5 - P.half_n1) * P.d, x2);
+                u1 = u.x; u2 = u.y;
                 finite = fabs(u1) <= 1.7976931348623157e308 && fabs(u2) <= 1.7976931348623157e308;
             }
             int pix;
@@ -469,138 +538,6 @@ float2 dx[kR / 2], r2[kR / 2], rc[kR / 2];
         if (tot) atomicAdd(&P.counters[3], tot);
     }
 }
-
-#ifdef MLENS_ABLATIONS
-// ---------------------------------------------------------------------------------------------------------------
-// ABLATION ONLY (mlens_set_option("kernel", 2)): the "obvious" FP32 kernel — Eq. (1) summed in plain FP32 in global
-// coordinates, same tiling, register blocking, packed arithmetic and MUFU reciprocal as the production kernel but no
-// difference form (5 packed FP32 instructions per ray pair instead of 6, no per-tile transform).  It exists to show
-// what the difference form buys: this kernel misses the north_star tolerances by 1-2 orders of magnitude
-// (tests/test_gpu_parity.py::test_plain_fp32_ablation_fails_the_tolerances).
-// ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(512, 2) shoot_plain_fp32_kernel(const ShootParams P) {
-    constexpr int kR = 8, kThreads = 512, kTx = kTile / kR;
-    extern __shared__ __align__(128) unsigned char smem_raw_bytes[];
-    float4* ls = reinterpret_cast<float4*>(smem_raw_bytes);  // whole lens list (x, y, m, 0), padded to a multiple of 4
-    const int tid = threadIdx.x, lane = tid & 31;
-    const int tx = tid % kTx, ty = tid / kTx;
-    const int n_pad = (P.n_lens + 3) & ~3;
-    for (int t = tid; t < n_pad; t += kThreads) ls[t] = t < P.n_lens ? P.lens_raw[t] : make_float4(kFar, kFar, 0.f, 0.f);
-    __syncthreads();
-    const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
-    unsigned long long c_in = 0, c_out = 0, c_lost = 0;
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const int tJ = (int)(tile / P.tiles_x), tI = (int)(tile - (long long)tJ * P.tiles_x);
-        const long long jray = P.j0 + (long long)tJ * kTile + ty;
-        const long long iray0 = P.i0 + (long long)tI * kTile + tx * kR;
-        const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
-        const float x2f = (float)x2;
-        float2 xf[kR / 2], ax[kR / 2], ay[kR / 2];
-#pragma unroll
-        for (int j = 0; j < kR / 2; ++j) {
-            xf[j].x = (float)(((double)(iray0 + 2 * j) + 0.5 - P.half_n1) * P.d);
-            xf[j].y = (float)(((double)(iray0 + 2 * j + 1) + 0.5 - P.half_n1) * P.d);
-            ax[j] = ay[j] = make_float2(0.f, 0.f);
-        }
-#pragma unroll 4
-        for (int l = 0; l < n_pad; ++l) {
-            const float4 q = ls[l];
-            const float dy = x2f - q.y, dy2 = dy * dy;
-            const float2 NX = make_float2(-q.x, -q.x), DY2 = make_float2(dy2, dy2), M = make_float2(q.z, q.z);
-            const float2 DY = make_float2(dy, dy);
-#pragma unroll
-            for (int j = 0; j < kR / 2; ++j) {
-                const float2 dx = __fadd2_rn(xf[j], NX);
-                const float2 r2 = __ffma2_rn(dx, dx, DY2);
-                const float2 w = __fmul2_rn(M, make_float2(rcp_mufu(r2.x), rcp_mufu(r2.y)));
-                ax[j] = __ffma2_rn(w, dx, ax[j]);
-                ay[j] = __ffma2_rn(w, DY, ay[j]);
-            }
-        }
-        int n_in = 0, n_out = 0, n_lost = 0;
-#pragma unroll
-        for (int k = 0; k < kR; ++k) {
-            const int j = k >> 1;
-            const long long iray = iray0 + k;
-            const bool ok = jray < P.j0 + P.nj && iray < P.i0 + P.ni;
-            const double x1 = ((double)iray + 0.5 - P.half_n1) * P.d;
-            const double y1 = P.f1 * x1 - (double)((k & 1) ? ax[j].y : ax[j].x);
-            const double y2 = P.f2 * x2 - (double)((k & 1) ? ay[j].y : ay[j].x);
-            int pix;
-            if (!(isfinite(y1) && isfinite(y2))) {
-                pix = -2;
-            } else {
-                const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
-                pix = (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
-                          ? (int)floor(u2) * P.npix + (int)floor(u1) : -1;
-            }
-            if (ok) {
-                n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
-                if (P.ray_y || P.ray_pix) {
-                    const long long qidx = (jray - P.j0) * P.ni + (iray - P.i0);
-                    if (P.ray_y) { P.ray_y[2 * qidx] = y1; P.ray_y[2 * qidx + 1] = y2; }
-                    if (P.ray_pix) P.ray_pix[qidx] = pix;
-                }
-                if (P.count && pix >= 0) red_add(P.count + pix, 1);
-            }
-        }
-        n_in = __reduce_add_sync(0xffffffffu, n_in);
-        n_out = __reduce_add_sync(0xffffffffu, n_out);
-        n_lost = __reduce_add_sync(0xffffffffu, n_lost);
-        c_in += n_in; c_out += n_out; c_lost += n_lost;
-    }
-    if (lane == 0) {
-        if (c_in) atomicAdd(&P.counters[0], c_in);
-        if (c_out) atomicAdd(&P.counters[1], c_out);
-        if (c_lost) atomicAdd(&P.counters[2], c_lost);
-        if (c_in + c_out + c_lost) atomicAdd(&P.counters[3], c_in + c_out + c_lost);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// plumbing / debug kernel: Eq. (1) in plain FP64, one ray per thread, lenses read from global memory
-// ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) shoot_fp64_kernel(const ShootParams P) {
-    const long long n_rays = P.ni * P.nj;
-    int n_in = 0, n_out = 0, n_lost = 0;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n_rays; q += (long long)gridDim.x * blockDim.x) {
-        const long long jj = q / P.ni, ii = q - jj * P.ni;
-        const double x1 = ((double)(P.i0 + ii) + 0.5 - P.half_n1) * P.d;
-        const double x2 = ((double)(P.j0 + jj) + 0.5 - P.half_n2) * P.d;
-        double a1 = 0.0, a2 = 0.0;
-        for (int k = 0; k < P.n_lens; ++k) {
-            const float4 l = __ldg(P.lens_raw + k);
-            const double dx = x1 - (double)l.x, dy = x2 - (double)l.y;
-            const double w = (double)l.z / (dx * dx + dy * dy);
-            a1 += w * dx;
-            a2 += w * dy;
-        }
-        const double y1 = P.f1 * x1 - a1, y2 = P.f2 * x2 - a2;
-        int pix;
-        if (!(isfinite(y1) && isfinite(y2))) {
-            pix = -2;
-        } else {
-            const double u1 = (y1 + P.half_L) / P.p, u2 = (y2 + P.half_L) / P.p;
-            pix = (u1 >= 0.0 && u1 < (double)P.npix && u2 >= 0.0 && u2 < (double)P.npix)
-                      ? (int)floor(u2) * P.npix + (int)floor(u1) : -1;
-        }
-        n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
-        if (P.ray_y) { P.ray_y[2 * q] = y1; P.ray_y[2 * q + 1] = y2; }
-        if (P.ray_pix) P.ray_pix[q] = pix;
-        if (P.count && pix >= 0) red_add(P.count + pix, 1);
-    }
-    n_in = __reduce_add_sync(0xffffffffu, n_in);
-    n_out = __reduce_add_sync(0xffffffffu, n_out);
-    n_lost = __reduce_add_sync(0xffffffffu, n_lost);
-    if ((threadIdx.x & 31) == 0) {
-        if (n_in) atomicAdd(&P.counters[0], (unsigned long long)n_in);
-        if (n_out) atomicAdd(&P.counters[1], (unsigned long long)n_out);
-        if (n_lost) atomicAdd(&P.counters[2], (unsigned long long)n_lost);
-        if (n_in + n_out + n_lost) atomicAdd(&P.counters[3], (unsigned long long)(n_in + n_out + n_lost));
-    }
-}
-
-#endif  // MLENS_ABLATIONS
 
 // ---------------------------------------------------------------------------------------------------------------
 // step a5 (Eq. 4): mag = (float)((double)count / N_avg); HBM-bound, 8 B per pixel

@@ -213,21 +213,42 @@ def test_binning_variants_and_fp64_kernel_agree(ml, oracle):
     assert np.abs(maps[1][0].astype(np.int64) - ref["count"]).sum() <= TOL_L1 * in_map
 
 
-@pytest.mark.parametrize("rays,shared", [(8, 0), (8, 1), (8, 2), (16, 0), (16, 1), (16, 2), (16, 4)])
-def test_shared_reciprocal_variants_meet_the_tolerances(ml, oracle, rays, shared):
-    # "shared_rcp": k of a thread's 4-ray groups per lens take 4 reciprocals from 2 MUFU.RCP; every setting must hold P10
+@pytest.mark.parametrize("tile_x,shared_pairs", [(64, 0), (64, 1), (64, 2), (64, 3), (64, 4), (48, 0), (48, 1), (48, 2), (32, 0),
+                                                 (32, 1), (32, 2)])
+def test_kernel_variants_meet_the_tolerances(ml, oracle, tile_x, shared_pairs):
+    # every instantiation of the production kernel's sweep grid (tile width x ray pairs per lens whose two reciprocals come
+    # from one MUFU.RCP) must hold P10; random + lens-centred blocks of cfg 4, ragged against all three tile widths
     cfg = fields.CONFIGS[4]
     xy, m = fields.lens_field(cfg)
     with ml.Mlens.from_config(cfg, xy, m, ablations=True) as h:
-        h.set_option("rays_per_thread", rays)
-        h.set_option("shared_rcp", shared)
+        h.set_option("tile_x", tile_x)
+        h.set_option("shared_pairs", shared_pairs)
         g = h.geometry
-        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 17, 3, 3, 0, size=192)
+        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 17, 3, 3, 0, size=200,
+                                   n_straddle=0, n_inside=2, map_half_image=cfg.map_half_image)
         tot = {"in_map": 0, "l1": 0}
         for b in blocks:
             r = check_block(ml, oracle, h, cfg, xy, m, b)
             tot["in_map"] += r["in_map"]; tot["l1"] += r["l1"]
-    assert tot["l1"] <= max(2, TOL_L1 * tot["in_map"]), tot
+    assert tot["in_map"] > 20000 and tot["l1"] <= max(2, TOL_L1 * tot["in_map"]), tot
+
+
+@pytest.mark.parametrize("shared", [0, 1])
+def test_round_1_kernel_still_meets_the_tolerances(ml, oracle, shared):
+    # "kernel" 4: the round-1 production kernel, kept in the ablations library as the A/B baseline of the timings
+    cfg = fields.CONFIGS[5]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m, ablations=True) as h:
+        h.set_option("kernel", 4)
+        h.set_option("shared_rcp", shared)
+        g = h.geometry
+        blocks = fields.block_plan(g.n1, g.n2, xy, cfg.half_widths, cfg.ray_spacing, cfg.seed + 19, 2, 2, 1, size=200,
+                                   n_straddle=0, n_inside=2, map_half_image=cfg.map_half_image)
+        tot = {"in_map": 0, "l1": 0}
+        for b in blocks:
+            r = check_block(ml, oracle, h, cfg, xy, m, b)
+            tot["in_map"] += r["in_map"]; tot["l1"] += r["l1"]
+    assert tot["in_map"] > 20000 and tot["l1"] <= max(2, TOL_L1 * tot["in_map"]), tot
 
 
 def test_near_list_overflow_falls_back_to_fp64(ml, oracle):
@@ -446,7 +467,7 @@ def test_shipped_library_refuses_the_ablation_kernels(ml):
     cfg = dataclasses.replace(fields.CONFIGS[1], npix=64, sub=2)
     xy, m = fields.lens_field(cfg)
     with ml.Mlens.from_config(cfg, xy, m) as h:
-        for key, value in (("kernel", 0), ("kernel", 2), ("kernel", 3), ("shared_rcp", 1), ("rays_per_thread", 16)):
+        for key, value in (("kernel", 0), ("kernel", 2), ("kernel", 3), ("kernel", 4), ("shared_rcp", 1)):
             with pytest.raises(ml.MlensError) as e:
                 h.set_option(key, value)
             assert e.value.code == ml.EINVAL
