@@ -147,6 +147,36 @@ int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_v
 int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* values_dev, int n_values, int* count_dev,
                       void* cuda_stream);
 
+/* Minimal-bit-width storage (PAPER.md:704-712 and Table B.6): "rather than using the standard 16-bit and 32-bit data
+ * types, we could define our own data types, using in each case the minimum required number of bits to represent a
+ * particular map" — for a ray-count map (bits from its largest count) or an indexed map (bits from n_distinct - 1).
+ *   mlens_bits_needed(v)      HOST helper: the smallest b >= 1 with v < 2^b (Table B.6: 16383 -> 14, 65535 -> 16,
+ *                             1048575 -> 20, 16777215 -> 24)
+ *   mlens_packed_words(n, b)  HOST helper: 32-bit words of a packed array of n b-bit values = ceil(n*b/32); -1 on bad
+ *                             arguments.  (A 10000^2 map at 14/16/20/22/24/32 bits: 167/191/238/262/286/381 MiB, Table B.6.)
+ *   mlens_pack_map            src_dev: DEVICE npix*npix values, 32-bit (int32 ray counts) or 16-bit (indexed map) as
+ *                             given by src_bits; packed_dev: DEVICE mlens_packed_words(npix*npix, bits) 32-bit words,
+ *                             caller-owned.  Value q occupies bits [q*bits, (q+1)*bits) of the little-endian bit stream
+ *                             (bit i of the stream is bit i%32 of word i/32).  Values are MASKED to `bits` bits: choose
+ *                             bits from mlens_bits_needed(max value).  1 <= bits <= src_bits.
+ *   mlens_unpack_map          the inverse, into 32-bit or 16-bit values (bits <= dst_bits).
+ * Integer-exact, asynchronous on `cuda_stream`.  MLENS_EINVAL for NULL pointers or widths outside those ranges. */
+int mlens_bits_needed(unsigned long long max_value);
+long long mlens_packed_words(long long n_values, int bits);
+int mlens_pack_map(mlens_t* h, const void* src_dev, int src_bits, int bits, unsigned int* packed_dev, void* cuda_stream);
+int mlens_unpack_map(mlens_t* h, const unsigned int* packed_dev, int bits, void* dst_dev, int dst_bits, void* cuda_stream);
+
+/* Re-binned view of the MPD (the tools bin the stored MPD "into a histogram before they are returned
+ * to the user.  By default, the number of bins is set to 100, with a maximum limit of 400").  Reading S20:
+ * n_out bins of equal width in log10(mu) on [mu_min, mu_max), mu = count / N_avg.
+ *   hist_dev   DEVICE n_bins unsigned 64-bit: the exact histogram written by mlens_mpd (unclamped: n_bins >= max_count+2)
+ *   prob_dev   DEVICE n_out doubles, caller-owned, zeroed by the call: prob[k] = (number of pixels with
+ *              floor(n_out*(log10(mu) - log10(mu_min))/(log10(mu_max) - log10(mu_min))) == k) / npix^2.  Pixels with
+ *              count 0 (mu = 0 has no logarithm) or mu outside [mu_min, mu_max) are left out, so sum(prob) <= 1.
+ * Asynchronous.  MLENS_EINVAL unless 1 <= n_out <= 400, n_bins >= 2 and 0 < mu_min < mu_max (finite). */
+int mlens_mpd_rebin(mlens_t* h, const unsigned long long* hist_dev, int n_bins, int n_out, double mu_min, double mu_max,
+                    double* prob_dev, void* cuda_stream);
+
 /* Finite-source convolution (Eq. 6): C = M * K = F^-1[F(M) F(K)].
  *
  * mlens_profile_kernel writes the convolution kernel K of a source profile: the profile is sampled at pixel centres

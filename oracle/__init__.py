@@ -196,3 +196,37 @@ def index_map(count):
     f.restype = ctypes.c_longlong
     n = f(_p(c, ctypes.c_int), ctypes.c_longlong(c.size), _p(values, ctypes.c_int), _p(indexed, ctypes.c_int))
     return values[:n].copy(), indexed
+
+
+def bits_needed(max_value: int) -> int:
+    """Smallest b >= 1 with max_value < 2**b (PAPER.md Table B.6)."""
+    f = lib().oracle_bits_needed
+    f.argtypes = [ctypes.c_ulonglong]
+    return int(f(int(max_value)))
+
+
+def pack_bits(values, bits: int):
+    """Minimal-bit-width bit stream of non-negative integers < 2**bits: uint32 words."""
+    v = np.ascontiguousarray(np.asarray(values).reshape(-1).astype(np.uint32))
+    n_words = (v.size * int(bits) + 31) // 32
+    packed = np.empty((n_words,), dtype=np.uint32)
+    lib().oracle_pack_bits(_p(v, ctypes.c_uint), ctypes.c_longlong(v.size), ctypes.c_int(int(bits)), _p(packed, ctypes.c_uint),
+                           ctypes.c_longlong(n_words))
+    return packed
+
+
+def unpack_bits(packed, n: int, bits: int):
+    pk = np.ascontiguousarray(np.asarray(packed, dtype=np.uint32).reshape(-1))
+    out = np.empty((int(n),), dtype=np.uint32)
+    lib().oracle_unpack_bits(_p(pk, ctypes.c_uint), ctypes.c_longlong(int(n)), ctypes.c_int(int(bits)), _p(out, ctypes.c_uint))
+    return out
+
+
+def mpd_rebin(hist, n_avg, n_pixels, n_out, mu_min, mu_max):
+    """Re-binned MPD (reading S20): float64 [n_out] probabilities in equal-width log10(mu) bins."""
+    h = np.ascontiguousarray(np.asarray(hist, dtype=np.uint64).reshape(-1))
+    prob = np.empty((int(n_out),), dtype=np.float64)
+    lib().oracle_mpd_rebin(_p(h, ctypes.c_ulonglong), ctypes.c_int(h.size), ctypes.c_double(float(n_avg)),
+                           ctypes.c_double(float(n_pixels)), ctypes.c_int(int(n_out)), ctypes.c_double(float(mu_min)),
+                           ctypes.c_double(float(mu_max)), _p(prob, ctypes.c_double))
+    return prob

@@ -288,6 +288,48 @@ long long oracle_index_map(const int* count, long long n_pixels, int* values, in
     return (long long)v.size();
 }
 
+// Minimal-bit-width storage (Table B.6).  Bit by bit, straight from the definition: bit k of value q
+// is bit q*bits + k of the stream, and bit i of the stream is bit i%32 of 32-bit word i/32.
+int oracle_bits_needed(unsigned long long max_value) {
+    int b = 1;
+    while (b < 64 && (max_value >> b) != 0ull) ++b;
+    return b;
+}
+
+void oracle_pack_bits(const unsigned int* values, long long n, int bits, unsigned int* packed, long long n_words) {
+    for (long long w = 0; w < n_words; ++w) packed[w] = 0u;
+    for (long long q = 0; q < n; ++q)
+        for (int k = 0; k < bits; ++k)
+            if ((values[q] >> k) & 1u) {
+                const long long i = q * bits + k;
+                packed[i >> 5] |= 1u << (i & 31);
+            }
+}
+
+void oracle_unpack_bits(const unsigned int* packed, long long n, int bits, unsigned int* values) {
+    for (long long q = 0; q < n; ++q) {
+        unsigned int v = 0u;
+        for (int k = 0; k < bits; ++k) {
+            const long long i = q * bits + k;
+            if ((packed[i >> 5] >> (i & 31)) & 1u) v |= 1u << k;
+        }
+        values[q] = v;
+    }
+}
+
+// Re-binned MPD (reading S20): n_out equal-width bins in log10(mu) on [mu_min, mu_max), one count
+// value at a time.
+void oracle_mpd_rebin(const unsigned long long* hist, int n_bins, double n_avg, double n_pixels, int n_out, double mu_min,
+                      double mu_max, double* prob) {
+    for (int k = 0; k < n_out; ++k) prob[k] = 0.0;
+    const double log_min = std::log10(mu_min), width = (std::log10(mu_max) - log_min) / n_out;
+    for (int c = 1; c < n_bins; ++c) {
+        if (!hist[c]) continue;
+        const double t = (std::log10((double)c / n_avg) - log_min) / width;
+        if (t >= 0.0 && t < (double)n_out) prob[(int)t] += (double)hist[c] / n_pixels;
+    }
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

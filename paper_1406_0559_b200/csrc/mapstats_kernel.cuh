@@ -29,16 +29,21 @@ struct MapStatsDev {               // device-side accumulator, zeroed (memset) b
 };
 
 // One pixel.  `lim` = min(smem_bins, n_bins-1): a single unsigned compare sends the common case (0 <= c < lim) to the
-// shared-memory bin; negative values (corrupt input -> bin 0), clamped counts (>= n_bins-1 -> last bin) and counts
-// beyond the shared-memory bins take the slow path.
+// shared-memory bin and does NOTHING else — the sum, minimum and maximum of those pixels are read off the finished
+// histogram by mpd_reduce_kernel (sum = sum_t t*hist[t], min/max = first/last non-empty bin), which takes a dozen
+// integer instructions per int4 out of the streaming loop.  Negative values (corrupt input -> bin 0), clamped counts
+// (>= n_bins-1 -> last bin) and counts beyond the shared-memory bins take the slow path, which keeps its own statistics.
 __device__ __forceinline__ void mpd_add(unsigned int* sh, unsigned lim, int smem_bins, unsigned long long* hist, int n_bins,
-                                        int c, unsigned long long& clamped) {
+                                        int c, unsigned long long& clamped, unsigned long long& sum, int& vmax, int& vmin) {
     if ((unsigned)c < lim) {
         atomicAdd(&sh[c], 1u);
     } else {
+        sum += (unsigned long long)(long long)c;
+        vmax = max(vmax, c);
+        vmin = min(vmin, c);
         int b = c < 0 ? 0 : c;
         if (b >= n_bins - 1) { b = n_bins - 1; ++clamped; }
-        if (b < smem_bins) atomicAdd(&sh[b], 1u);
+        if (b < smem_bins) atomicAdd(&sh[b], 1u);  // only the slow path puts pixels into shared bins >= lim (the last bin)
         else atomicAdd(&hist[b], 1ull);
     }
 }
@@ -77,18 +82,13 @@ __global__ void __launch_bounds__(kMpdThreads, 1) mpd_kernel(const int* __restri
             // one add of 128.  Elsewhere neighbouring counts differ (Poisson-like scatter) and conflicts are rare.
             const int w0 = __shfl_sync(0xffffffffu, w.x, 0);
             const bool flat = __all_sync(0xffffffffu, ok[u] && w.x == w0 && w.y == w0 && w.z == w0 && w.w == w0);
-            if (ok[u]) {
-                sum += (unsigned long long)((long long)w.x + w.y + w.z + w.w);
-                vmax = max(max(vmax, max(w.x, w.y)), max(w.z, w.w));
-                vmin = min(min(vmin, min(w.x, w.y)), min(w.z, w.w));
-            }
             if (flat && (unsigned)w0 < lim) {
                 if ((threadIdx.x & 31) == 0) atomicAdd(&sh[w0], 128u);
             } else if (ok[u]) {
-                mpd_add(sh, lim, smem_bins, hist, n_bins, w.x, clamped);
-                mpd_add(sh, lim, smem_bins, hist, n_bins, w.y, clamped);
-                mpd_add(sh, lim, smem_bins, hist, n_bins, w.z, clamped);
-                mpd_add(sh, lim, smem_bins, hist, n_bins, w.w, clamped);
+                mpd_add(sh, lim, smem_bins, hist, n_bins, w.x, clamped, sum, vmax, vmin);
+                mpd_add(sh, lim, smem_bins, hist, n_bins, w.y, clamped, sum, vmax, vmin);
+                mpd_add(sh, lim, smem_bins, hist, n_bins, w.z, clamped, sum, vmax, vmin);
+                mpd_add(sh, lim, smem_bins, hist, n_bins, w.w, clamped, sum, vmax, vmin);
             }
         }
     }
@@ -122,8 +122,11 @@ __global__ void __launch_bounds__(kMpdThreads, 1) mpd_kernel(const int* __restri
 // hist[t] += sum over CTAs of partial[cta][t].  32 bins x 8 slice-groups per 256-thread block: reads are coalesced
 // across the 32 bins, every thread has ~n_ctas/8 independent loads (a single thread walking all 148 slices is
 // latency-bound: ~90 us), no contended atomics.
+// The statistics of the fast-path pixels (count < lim = min(smem_bins, n_bins-1)) come from here: bin t holds v pixels of
+// count t, so they add t*v to the sum and, if v > 0, make t a candidate for the minimum and the maximum.
 __global__ void __launch_bounds__(256) mpd_reduce_kernel(const unsigned int* __restrict__ partial, int n_ctas, int smem_bins,
-                                                         unsigned long long* __restrict__ hist, int n_bins) {
+                                                         unsigned long long* __restrict__ hist, int n_bins,
+                                                         MapStatsDev* __restrict__ out) {
     __shared__ unsigned long long part[8][32];
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
     const int t = blockIdx.x * 32 + tx;
@@ -138,6 +141,20 @@ __global__ void __launch_bounds__(256) mpd_reduce_kernel(const unsigned int* __r
 #pragma unroll
         for (int k = 1; k < 8; ++k) v += part[k][tx];
         if (v) atomicAdd(&hist[t], v);  // ragged-tail pixels and counts >= smem_bins were added atomically by mpd_kernel
+    }
+    if (ty == 0) {  // warp 0: statistics of the fast-path bins of this block
+        const bool fast = t < min(smem_bins, n_bins - 1);
+        unsigned long long s = fast ? v * (unsigned long long)t : 0ull;
+        int lo = (fast && v) ? t : 0x7fffffff, hi = (fast && v) ? t : 0;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+        lo = __reduce_min_sync(0xffffffffu, lo);
+        hi = __reduce_max_sync(0xffffffffu, hi);
+        if (tx == 0) {
+            if (s) atomicAdd(&out->sum_count, s);
+            if (hi > 0) atomicMax(&out->max_count, hi);
+            if (lo != 0x7fffffff) atomicMax(&out->inv_min_count, 0x7fffffff - lo);
+        }
     }
 }
 
@@ -225,6 +242,66 @@ __global__ void __launch_bounds__(256) index_decode_kernel(const unsigned short*
     }
     for (long long q = (n4 << 2) + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride)
         count[q] = indexed[q] < n_values ? __ldg(values + indexed[q]) : -1;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Minimal-bit-width storage (Table B.6): "rather than using the standard 16-bit and 32-bit data
+// types, we could define our own data types, using in each case the minimum required number of bits to represent a
+// particular map".  Value q (masked to `bits` bits) occupies bits [q*bits, (q+1)*bits) of a little-endian bit stream
+// held in 32-bit words.  HBM-bound: src bytes in, bits/8 bytes out per value.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename SrcT>
+__global__ void __launch_bounds__(256) pack_bits_kernel(const SrcT* __restrict__ src, long long n, int bits,
+                                                        unsigned int* __restrict__ packed, long long n_words) {
+    const unsigned long long mask = bits >= 32 ? 0xffffffffull : ((1ull << bits) - 1ull);
+    const long long stride = (long long)gridDim.x * 256;
+    for (long long w = (long long)blockIdx.x * 256 + threadIdx.x; w < n_words; w += stride) {  // one output word each
+        const long long bit0 = w << 5;
+        long long q = bit0 / bits;
+        int off = (int)(bit0 - q * bits);  // bits of value q that already went into the previous word
+        unsigned int acc = 0u;
+        int filled = 0;
+        while (filled < 32 && q < n) {
+            const unsigned long long v = (unsigned long long)(unsigned int)src[q] & mask;
+            acc |= (unsigned int)((v >> off) << filled);
+            filled += bits - off;
+            off = 0;
+            ++q;
+        }
+        packed[w] = acc;
+    }
+}
+
+template <typename DstT>
+__global__ void __launch_bounds__(256) unpack_bits_kernel(const unsigned int* __restrict__ packed, long long n, int bits,
+                                                          DstT* __restrict__ dst) {
+    const unsigned long long mask = bits >= 32 ? 0xffffffffull : ((1ull << bits) - 1ull);
+    const long long stride = (long long)gridDim.x * 256;
+    for (long long q = (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride) {
+        const long long bit0 = q * bits;
+        const long long w = bit0 >> 5;
+        const int sh = (int)(bit0 & 31);
+        unsigned long long window = (unsigned long long)__ldg(packed + w);
+        if (sh + bits > 32) window |= (unsigned long long)__ldg(packed + w + 1) << 32;
+        dst[q] = (DstT)((window >> sh) & mask);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Re-binned view of the MPD (the tools bin mpd.dat "into a histogram before they are returned ... By
+// default, the number of bins is set to 100, with a maximum limit of 400").  Reading S20: n_out bins of
+// equal width in log10(mu) on [mu_min, mu_max), mu = count/N_avg; out[k] = (pixels whose mu falls in bin k)/n_pixels;
+// count 0 (mu = 0) and magnifications outside the range are left out.  One thread per exact-histogram bin.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) mpd_rebin_kernel(const unsigned long long* __restrict__ hist, int n_bins, double n_avg,
+                                                        double n_pixels, int n_out, double log_min, double inv_width,
+                                                        double* __restrict__ out) {
+    for (int c = 1 + blockIdx.x * 256 + threadIdx.x; c < n_bins; c += gridDim.x * 256) {
+        const unsigned long long hcount = hist[c];
+        if (hcount == 0ull) continue;
+        const double t = (log10((double)c / n_avg) - log_min) * inv_width;
+        if (t >= 0.0 && t < (double)n_out) atomicAdd(out + (int)t, (double)hcount / n_pixels);
+    }
 }
 
 }  // namespace mlk

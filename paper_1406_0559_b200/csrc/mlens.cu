@@ -49,11 +49,14 @@ constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chun
 #ifndef MLENS_PROD_TILE_X
 #define MLENS_PROD_TILE_X 64
 #endif
-#ifndef MLENS_PROD_SHARED_PAIRS
-#define MLENS_PROD_SHARED_PAIRS 0
+#ifndef MLENS_PROD_RAYS
+#define MLENS_PROD_RAYS 16
 #endif
-constexpr int kProdTileX = MLENS_PROD_TILE_X, kProdSharedPairs = MLENS_PROD_SHARED_PAIRS;
-constexpr int kProdCtas = kProdTileX == 32 ? 3 : 2;
+#ifndef MLENS_PROD_SHARED_PAIRS
+#define MLENS_PROD_SHARED_PAIRS 2
+#endif
+constexpr int kProdTileX = MLENS_PROD_TILE_X, kProdRays = MLENS_PROD_RAYS, kProdSharedPairs = MLENS_PROD_SHARED_PAIRS;
+constexpr int kProdCtas = 2;
 constexpr int kTileCtrSlots = 256;     // ring of dynamic tile counters: one per launch in flight (see launch_block)
 
 }  // namespace
@@ -230,26 +233,27 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         int shared = h->opt_shared_pairs;
         const double zmax = (h->lens_extent + std::fmax(h->geo.a1, h->geo.a2)) / h->d;  // per axis, lattice units
         if (shared > 0 && 4.0 * zmax * zmax * zmax * zmax > 1.0e37) shared = 0;
-        const int code = h->opt_tile_x * 10 + shared;
+        const int code = h->opt_rays * 10000 + h->opt_tile_x * 10 + shared;
         const bool runs = h->opt_binning == mlk::BIN_RUNS;  // the default binning route is compiled in (shorter epilogue)
         switch (code) {
-#define MLENS_VARIANT(TX, SP, NC)                                                                        \
-    case TX * 10 + SP:                                                                                   \
-        kern = runs ? mlk::shoot_fp32_kernel<TX, 8, SP, NC, mlk::BIN_RUNS> : mlk::shoot_fp32_kernel<TX, 8, SP, NC, -1>; \
-        threads = TX / 8 * mlk::kTile; ctas = NC;                                                        \
+#define MLENS_VARIANT(TX, R, SP, NC)                                                                                       \
+    case R * 10000 + TX * 10 + SP:                                                                                          \
+        kern = runs ? mlk::shoot_fp32_kernel<TX, R, SP, NC, mlk::BIN_RUNS> : mlk::shoot_fp32_kernel<TX, R, SP, NC, -1>;     \
+        threads = TX / R * mlk::kTile; ctas = NC;                                                                           \
         break;
-#ifdef MLENS_ABLATIONS  // the whole sweep grid: tile width x shared pairs
-#define MLENS_SWEEP(SP) MLENS_VARIANT(64, SP, 2) MLENS_VARIANT(48, SP, 2) MLENS_VARIANT(32, SP, 3)
-            MLENS_SWEEP(0) MLENS_SWEEP(1) MLENS_SWEEP(2) MLENS_VARIANT(64, 3, 2) MLENS_VARIANT(64, 4, 2)
+#ifdef MLENS_ABLATIONS  // the sweep grid: rays per thread x tile width x shared pairs (profiles/)
+#define MLENS_SWEEP(SP) MLENS_VARIANT(64, 8, SP, 2) MLENS_VARIANT(48, 8, SP, 2) MLENS_VARIANT(32, 8, SP, 3) MLENS_VARIANT(64, 16, SP, 2)
+            MLENS_SWEEP(0) MLENS_SWEEP(1) MLENS_SWEEP(2)
+            MLENS_VARIANT(64, 8, 3, 2) MLENS_VARIANT(64, 8, 4, 2) MLENS_VARIANT(64, 16, 3, 2) MLENS_VARIANT(64, 16, 4, 2)
 #undef MLENS_SWEEP
 #else                   // the shipped library: the production instantiation and its one-reciprocal-per-ray fallback
-            MLENS_VARIANT(kProdTileX, 0, kProdCtas)
+            MLENS_VARIANT(kProdTileX, kProdRays, 0, kProdCtas)
 #if MLENS_PROD_SHARED_PAIRS != 0
-            MLENS_VARIANT(kProdTileX, kProdSharedPairs, kProdCtas)
+            MLENS_VARIANT(kProdTileX, kProdRays, kProdSharedPairs, kProdCtas)
 #endif
 #endif
 #undef MLENS_VARIANT
-            default: return fail(MLENS_EINVAL, "no kernel variant tile_x=%d shared_pairs=%d in this build", h->opt_tile_x, shared);
+            default: return fail(MLENS_EINVAL, "no kernel variant rays_per_thread=%d tile_x=%d shared_pairs=%d in this build", h->opt_rays, h->opt_tile_x, shared);
         }
     }
     if (h->opt_ctas_per_sm > 0) ctas = h->opt_ctas_per_sm;
@@ -351,7 +355,7 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
     h->npix = npix; h->n_lens = n_lens; h->geo = g;
     h->device = dev; h->sm_count = prop.multiProcessorCount;
-    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 0; h->opt_shared = 0; h->opt_rays = 8;
+    h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 0; h->opt_shared = 0; h->opt_rays = kProdRays;
     h->opt_tile_x = kProdTileX; h->opt_shared_pairs = kProdSharedPairs;
     for (long long k = 0; k < n_lens; ++k)
         h->lens_extent = std::fmax(h->lens_extent, std::fmax(std::fabs((double)packed[(size_t)k].x), std::fabs((double)packed[(size_t)k].y)));
@@ -419,7 +423,7 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
     // the shipped library holds the production kernel only: the debug / ablation / experimental kernels and loop variants
     // exist in the MLENS_ABLATIONS build (libmlens_ablations.so, used by the tests and the profiling runs)
     if ((!strcmp(key, "kernel") && value != 1) || (!strcmp(key, "shared_rcp") && value != 0) ||
-        (!strcmp(key, "tile_x") && value != kProdTileX) ||
+        (!strcmp(key, "tile_x") && value != kProdTileX) || (!strcmp(key, "rays_per_thread") && value != kProdRays) ||
         (!strcmp(key, "shared_pairs") && value != 0 && value != kProdSharedPairs))
         return fail(MLENS_EINVAL, "option %s=%lld needs the MLENS_ABLATIONS build of the library", key, value);
 #endif
@@ -429,6 +433,9 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
     } else if (!strcmp(key, "tile_x")) {
         if (value != 64 && value != 48 && value != 32) return fail(MLENS_EINVAL, "tile_x must be 64, 48 or 32");
         h->opt_tile_x = (int)value;
+    } else if (!strcmp(key, "rays_per_thread")) {
+        if (value != 8 && value != 16) return fail(MLENS_EINVAL, "rays_per_thread must be 8 or 16");
+        h->opt_rays = (int)value;
     } else if (!strcmp(key, "shared_pairs")) {
         if (value < 0 || value > 4) return fail(MLENS_EINVAL, "shared_pairs must be 0..4");
         h->opt_shared_pairs = (int)value;
@@ -498,7 +505,7 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
     mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n, hist_dev, n_bins, smem_bins,
                                                                        h->mpd_partial, h->mapstats_dev);
     MLENS_CUDA(cudaGetLastError());
-    mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(h->mpd_partial, (int)blocks, smem_bins, hist_dev, n_bins);
+    mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(h->mpd_partial, (int)blocks, smem_bins, hist_dev, n_bins, h->mapstats_dev);
     MLENS_CUDA(cudaGetLastError());
     if (stats) {
         MLENS_CUDA(cudaMemcpyAsync(h->mapstats_host, h->mapstats_dev, sizeof(mlk::MapStatsDev), cudaMemcpyDeviceToHost, st));
@@ -569,6 +576,68 @@ int mlens_unindex_map(mlens_t* h, const unsigned short* indexed_dev, const int* 
     if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
     if (blocks < 1) blocks = 1;
     mlk::index_decode_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(indexed_dev, n, values_dev, n_values, count_dev);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int mlens_bits_needed(unsigned long long max_value) {
+    int b = 1;
+    while (b < 64 && (max_value >> b) != 0ull) ++b;
+    return b;
+}
+
+long long mlens_packed_words(long long n_values, int bits) {
+    if (n_values < 0 || bits < 1 || bits > 32) return -1;
+    return (n_values * bits + 31) / 32;
+}
+
+int mlens_pack_map(mlens_t* h, const void* src_dev, int src_bits, int bits, unsigned int* packed_dev, void* cuda_stream) {
+    if (!h || !src_dev || !packed_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
+    if (src_bits != 16 && src_bits != 32) return fail(MLENS_EINVAL, "src_bits must be 16 or 32");
+    if (bits < 1 || bits > src_bits) return fail(MLENS_EINVAL, "bits must be 1..src_bits");
+    const long long n = (long long)h->npix * h->npix, n_words = mlens_packed_words(n, bits);
+    long long blocks = (n_words + 255) / 256;
+    if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
+    if (src_bits == 32)
+        mlk::pack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const int*)src_dev, n, bits, packed_dev, n_words);
+    else
+        mlk::pack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned short*)src_dev, n, bits, packed_dev, n_words);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int mlens_unpack_map(mlens_t* h, const unsigned int* packed_dev, int bits, void* dst_dev, int dst_bits, void* cuda_stream) {
+    if (!h || !packed_dev || !dst_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
+    if (dst_bits != 16 && dst_bits != 32) return fail(MLENS_EINVAL, "dst_bits must be 16 or 32");
+    if (bits < 1 || bits > dst_bits) return fail(MLENS_EINVAL, "bits must be 1..dst_bits");
+    const long long n = (long long)h->npix * h->npix;
+    long long blocks = (n + 255) / 256;
+    if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
+    if (dst_bits == 32)
+        mlk::unpack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (int*)dst_dev);
+    else
+        mlk::unpack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (unsigned short*)dst_dev);
+    MLENS_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+int mlens_mpd_rebin(mlens_t* h, const unsigned long long* hist_dev, int n_bins, int n_out, double mu_min, double mu_max,
+                    double* prob_dev, void* cuda_stream) {
+    if (!h || !hist_dev || !prob_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
+    if (n_bins < 2) return fail(MLENS_EINVAL, "n_bins must be >= 2");
+    if (n_out < 1 || n_out > 400) return fail(MLENS_EINVAL, "n_out must be 1..400 (PAPER.md:453: 'a maximum limit of 400')");
+    if (!std::isfinite(mu_min) || !std::isfinite(mu_max) || !(mu_min > 0) || !(mu_max > mu_min))
+        return fail(MLENS_EINVAL, "0 < mu_min < mu_max required");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    MLENS_CUDA(cudaMemsetAsync(prob_dev, 0, sizeof(double) * (size_t)n_out, st));
+    const double log_min = std::log10(mu_min), inv_width = (double)n_out / (std::log10(mu_max) - log_min);
+    int blocks = (n_bins + 255) / 256;
+    if (blocks > h->sm_count * 8) blocks = h->sm_count * 8;
+    mlk::mpd_rebin_kernel<<<blocks, 256, 0, st>>>(hist_dev, n_bins, h->geo.n_avg, (double)h->npix * (double)h->npix, n_out, log_min,
+                                                   inv_width, prob_dev);
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }

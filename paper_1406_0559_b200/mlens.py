@@ -70,6 +70,12 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_mpd.argtypes = [vp, vp, vp, ci, vp, ctypes.POINTER(MapStats)]
     L.mlens_index_map.argtypes = [vp, vp, vp, ci, vp, vp, ctypes.POINTER(ci)]
     L.mlens_unindex_map.argtypes = [vp, vp, vp, ci, vp, vp]
+    L.mlens_bits_needed.argtypes = [ctypes.c_ulonglong]
+    L.mlens_packed_words.argtypes = [ll, ci]
+    L.mlens_packed_words.restype = ll
+    L.mlens_pack_map.argtypes = [vp, vp, ci, ci, vp, vp]
+    L.mlens_unpack_map.argtypes = [vp, vp, ci, vp, ci, vp]
+    L.mlens_mpd_rebin.argtypes = [vp, vp, ci, ci, dbl, dbl, vp, vp]
     L.mlens_profile_kernel.argtypes = [vp, ci, dbl, vp, vp]
     L.mlens_convolve.argtypes = [vp, vp, vp, vp, vp]
     L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
@@ -82,7 +88,8 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_destroy.restype = None
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
                  "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
-                 "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option"):
+                 "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option", "mlens_bits_needed",
+                 "mlens_pack_map", "mlens_unpack_map", "mlens_mpd_rebin"):
         getattr(L, name).restype = ci
     _libs[key] = L
     return L
@@ -236,6 +243,40 @@ class Mlens:
         self._ck(self._L.mlens_unindex_map(self._h, ctypes.c_void_p(indexed.data_ptr()), ctypes.c_void_p(values.data_ptr()),
                                        int(values.numel()), ctypes.c_void_p(count.data_ptr()), _stream_ptr(stream)))
         return count
+
+    def pack_map(self, src, bits: int, stream=None):
+        """mlens_pack_map: int32 or uint16 map -> uint32 words of the `bits`-per-value bit stream."""
+        import torch
+
+        assert src.is_cuda and src.is_contiguous() and src.numel() == self.npix**2 and src.dtype in (torch.int32, torch.uint16)
+        n_words = int(self._L.mlens_packed_words(self.npix**2, int(bits)))
+        if n_words < 0:
+            raise MlensError(EINVAL, "bits must be 1..32")
+        packed = torch.empty((n_words,), dtype=torch.int32, device="cuda")  # 32-bit words (torch views them as int32)
+        self._ck(self._L.mlens_pack_map(self._h, ctypes.c_void_p(src.data_ptr()), 32 if src.dtype == torch.int32 else 16, int(bits),
+                                        ctypes.c_void_p(packed.data_ptr()), _stream_ptr(stream)))
+        return packed
+
+    def unpack_map(self, packed, bits: int, dtype=None, stream=None):
+        """mlens_unpack_map: the inverse of pack_map, into int32 (default) or uint16."""
+        import torch
+
+        dtype = dtype or torch.int32
+        assert packed.is_cuda and packed.is_contiguous() and packed.dtype == torch.int32 and dtype in (torch.int32, torch.uint16)
+        dst = torch.empty((self.npix, self.npix), dtype=dtype, device="cuda")
+        self._ck(self._L.mlens_unpack_map(self._h, ctypes.c_void_p(packed.data_ptr()), int(bits), ctypes.c_void_p(dst.data_ptr()),
+                                          32 if dtype == torch.int32 else 16, _stream_ptr(stream)))
+        return dst
+
+    def mpd_rebin(self, hist, n_out: int, mu_min: float, mu_max: float, stream=None):
+        """mlens_mpd_rebin: the exact MPD histogram -> n_out (<= 400) bins of equal width in log10(mu); float64 [n_out]."""
+        import torch
+
+        assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous()
+        prob = torch.empty((int(n_out),), dtype=torch.float64, device="cuda")
+        self._ck(self._L.mlens_mpd_rebin(self._h, ctypes.c_void_p(hist.data_ptr()), int(hist.numel()), int(n_out), float(mu_min),
+                                         float(mu_max), ctypes.c_void_p(prob.data_ptr()), _stream_ptr(stream)))
+        return prob
 
     def profile_kernel(self, shape: int, size_pixels: float, kernel=None, stream=None):
         """mlens_profile_kernel: convolution kernel of a source profile (0 uniform disc, 1 Gaussian), float32 [npix,npix]."""

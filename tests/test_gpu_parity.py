@@ -213,14 +213,16 @@ def test_binning_variants_and_fp64_kernel_agree(ml, oracle):
     assert np.abs(maps[1][0].astype(np.int64) - ref["count"]).sum() <= TOL_L1 * in_map
 
 
-@pytest.mark.parametrize("tile_x,shared_pairs", [(64, 0), (64, 1), (64, 2), (64, 3), (64, 4), (48, 0), (48, 1), (48, 2), (32, 0),
-                                                 (32, 1), (32, 2)])
-def test_kernel_variants_meet_the_tolerances(ml, oracle, tile_x, shared_pairs):
-    # every instantiation of the production kernel's sweep grid (tile width x ray pairs per lens whose two reciprocals come
-    # from one MUFU.RCP) must hold P10; random + lens-centred blocks of cfg 4, ragged against all three tile widths
+@pytest.mark.parametrize("rays,tile_x,shared_pairs", [(16, 64, 0), (16, 64, 1), (16, 64, 2), (16, 64, 3), (16, 64, 4), (8, 64, 0),
+                                                      (8, 64, 1), (8, 64, 2), (8, 64, 4), (8, 48, 0), (8, 48, 2), (8, 32, 1)])
+def test_kernel_variants_meet_the_tolerances(ml, oracle, rays, tile_x, shared_pairs):
+    # every instantiation of the production kernel's sweep grid (rays per thread x tile width x ray pairs per lens whose two
+    # reciprocals come from one MUFU.RCP) must hold P10; random + lens-centred + in-map blocks of cfg 4, ragged against all
+    # three tile widths
     cfg = fields.CONFIGS[4]
     xy, m = fields.lens_field(cfg)
     with ml.Mlens.from_config(cfg, xy, m, ablations=True) as h:
+        h.set_option("rays_per_thread", rays)
         h.set_option("tile_x", tile_x)
         h.set_option("shared_pairs", shared_pairs)
         g = h.geometry
@@ -231,6 +233,24 @@ def test_kernel_variants_meet_the_tolerances(ml, oracle, tile_x, shared_pairs):
             r = check_block(ml, oracle, h, cfg, xy, m, b)
             tot["in_map"] += r["in_map"]; tot["l1"] += r["l1"]
     assert tot["in_map"] > 20000 and tot["l1"] <= max(2, TOL_L1 * tot["in_map"]), tot
+
+
+def test_far_lens_and_tiny_spacing_take_the_one_reciprocal_path(ml, oracle):
+    # shared reciprocals multiply two squared distances in lattice units (lengths / d): a lens 2e4 R_E away with d = 1e-6
+    # gives r^2 ~ 4e20 and a product beyond FP32, so the library must fall back to one MUFU.RCP per ray — and still match
+    L, npix = 1.0e-3, 16
+    d = 1.0e-6
+    xy = np.array([[20000.0, 5000.0], [-3.0, 1.0], [0.5, -0.25]], np.float32)
+    m = np.array([4.0, 1.0, 0.5], np.float32)
+    cfg = fields.MapConfig("far", npix, L, 0.3, 0.1, 0.0, 1, "unit", 0)
+    with ml.Mlens(0.3, 0.1, 0.0, L, npix, d, xy, m) as h:
+        g = h.geometry
+        for b in [(0, 0, 130, 70), (g.n1 // 2 - 100, g.n2 // 2 - 100, 200, 200)]:
+            i0, j0, ni, nj = b
+            out = h.shoot_block(i0, j0, ni, nj, want_rays=True)
+            ref = oracle.shoot_block(0.3, 0.1, 0.0, L, npix, d, xy, m, block=b, want_rays=True)
+            assert np.abs(out["y"].cpu().numpy() - ref["y"]).max() <= 2e-5 * ref["scale"].min()
+            assert (out["pix"].cpu().numpy() != ref["pix"]).sum() <= 2
 
 
 @pytest.mark.parametrize("shared", [0, 1])
@@ -467,7 +487,8 @@ def test_shipped_library_refuses_the_ablation_kernels(ml):
     cfg = dataclasses.replace(fields.CONFIGS[1], npix=64, sub=2)
     xy, m = fields.lens_field(cfg)
     with ml.Mlens.from_config(cfg, xy, m) as h:
-        for key, value in (("kernel", 0), ("kernel", 2), ("kernel", 3), ("kernel", 4), ("shared_rcp", 1)):
+        for key, value in (("kernel", 0), ("kernel", 2), ("kernel", 3), ("kernel", 4), ("shared_rcp", 1), ("rays_per_thread", 8),
+                           ("tile_x", 48), ("shared_pairs", 1)):
             with pytest.raises(ml.MlensError) as e:
                 h.set_option(key, value)
             assert e.value.code == ml.EINVAL
