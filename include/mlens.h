@@ -210,15 +210,19 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream);
 /* Tuning switches.  Keys of the shipped library (libmlens.so):
  *   "binning"      0 = one global RED per ray, 1 = per-thread run-combine (default), 2 = + warp aggregation,
  *                  3 = + CTA-private shared-memory window — four routes to the same map, bit-identical results
- *   "ctas_per_sm"  persistent CTAs per SM (default 2)
- *   "kernel"       1 = the production FP32 difference-form kernel (the only value the shipped library accepts)
- * The debug / ablation / experimental kernels are compiled only with -DMLENS_ABLATIONS (libmlens_ablations.so, which
- * the tests and profiling runs load; the shipped library returns MLENS_EINVAL for them, so the public ABI cannot
- * select a kernel that misses the parity tolerances):
+ *   "ctas_per_sm"  persistent CTAs per SM; 0 (default) = the kernel's own choice (2)
+ *   "shared_pairs" ray pairs per lens (of a thread's 8) whose reciprocals are shared: 2 (default) or 0 (one MUFU.RCP per
+ *                  ray; also chosen automatically when lens coordinates / ray_spacing would overflow the FP32 products)
+ *   "kernel" = 1, "rays_per_thread" = 16, "tile_x" = 64: accepted with these (production) values only
+ * The debug / ablation / experimental kernels and the sweep grid are compiled only with -DMLENS_ABLATIONS
+ * (libmlens_ablations.so, which the tests and profiling runs load; the shipped library returns MLENS_EINVAL for them, so
+ * the public ABI cannot select a kernel that misses the parity tolerances):
  *   "kernel"       0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 2 = plain-form FP32 kernel (does NOT meet
  *                  the parity tolerances: the evidence for the difference form; <= 12000 lenses), 3 = tensor-pipe
- *                  experiment (r^2, Re, Im of every interaction from tcgen05 TF32 MMAs; slower than kernel 1)
- *   "shared_rcp", "rays_per_thread"   loop variants of kernel 1
+ *                  experiment (r^2, Re, Im of every interaction from tcgen05 TF32 MMAs; slower than kernel 1 and NOT
+ *                  deterministic: its per-ray partial sums meet in shared-memory float atomics), 4 = the round-1
+ *                  production kernel (A/B baseline; its loop variant "shared_rcp" 0..2)
+ *   "rays_per_thread" 8 | 16, "tile_x" 64 | 48 | 32 (8 rays only), "shared_pairs" 0..4: the sweep grid of kernel 1
  * Returns MLENS_EINVAL for an unknown key or value. */
 int mlens_set_option(mlens_t* h, const char* key, long long value);
 
