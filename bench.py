@@ -337,6 +337,7 @@ def run_ours(args):
     e2e_steps = max(1, min(args.steps, 2))
     h.close()
     barrier()
+    e2e_kernel_ms = []
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         with mlens.Mlens.from_config(cfg, xy, m) as h2:
@@ -345,6 +346,7 @@ def run_ours(args):
                 c_host, m_host = c_dev.cpu().numpy(), m_dev.cpu().numpy()
             else:
                 c_host, m_host, st2 = h2.shoot_host()
+            e2e_kernel_ms.append(st2.get("kernel_ms"))
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -361,6 +363,7 @@ def run_ours(args):
                          clocks=clocks, sms=prop.multi_processor_count, e2e_s=e2e_s, e2e_steps=e2e_steps,
                          h2d_bytes=xy.nbytes + m.nbytes, d2h_bytes=c_host.nbytes + m_host.nbytes, peak_meas=peak_meas,
                          traffic=traffic, traffic_source=traffic_source)
+        line["e2e"]["kernel_ms_per_step"] = e2e_kernel_ms  # of which: the shooting kernel (events inside libmlens)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = run_cpu_baseline(cfg, xy, m)
         print(json.dumps(line), flush=True)

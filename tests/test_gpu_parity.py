@@ -419,6 +419,24 @@ def test_config_1_full_map_against_the_oracle(ml, oracle):
     assert np.array_equal(mag, oracle.magnification(count.astype(np.int32), g.n_avg))
 
 
+def test_whole_lattice_production_kernel_against_the_fp64_kernel(ml):
+    # CUDA against CUDA, so no parity credit — but it is the one affordable check that NO tile position of a whole
+    # multi-million-tile lattice misbehaves: cfg 3's full map (9.7e9 rays, 2.4e6 tiles) through the production kernel and
+    # through the plain FP64 one-ray-per-thread kernel (itself held to 1e-6 of the oracle on small maps, above)
+    cfg = fields.CONFIGS[3]
+    xy, m = fields.lens_field(cfg)
+    with ml.Mlens.from_config(cfg, xy, m, ablations=True) as h:
+        a, _, sa = h.shoot(want_mag=False)
+        a = a.clone()
+        h.set_option("kernel", 0)
+        b, _, sb = h.shoot(want_mag=False)
+        l1 = int((a.to(torch.int64) - b.to(torch.int64)).abs().sum().item())
+    print(f"cfg3 whole lattice: production {sa['elapsed_ms']:.0f} ms, FP64 kernel {sb['elapsed_ms']:.0f} ms, in_map {sa['rays_in_map']} / "
+          f"{sb['rays_in_map']}, L1 {l1} ({l1 / sb['rays_in_map']:.2e})")
+    assert sa["rays_total"] == sb["rays_total"] == 196608 * 49152 and sa["rays_lost"] == sb["rays_lost"]
+    assert l1 <= TOL_L1 * sb["rays_in_map"] and abs(sa["rays_in_map"] - sb["rays_in_map"]) <= l1
+
+
 @pytest.mark.parametrize("cfg_id", [1, 3, 4, 5])
 def test_tensor_pipe_kernel_meets_the_tolerances(ml, oracle, cfg_id):
     # "kernel" 3 (experimental): r^2, Re, Im of every interaction from one tcgen05 TF32 MMA per 128 rays x 64 lenses, shared
