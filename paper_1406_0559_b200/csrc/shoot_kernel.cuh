@@ -397,7 +397,6 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
         float sre[kR], sim[kR];
 #pragma unroll
         for (int k = 0; k < kR; ++k) {
-            constexpr int kDummy = 0; (void)kDummy;
             const int j = RayMap<kR>::pair_of(k);
             const bool hi = RayMap<kR>::hi_of(k);
             const float eps = (float)k - 0.5f * (float)(kR - 1);
