@@ -194,8 +194,14 @@ int mlens_mpd_rebin(mlens_t* h, const unsigned long long* hist_dev, int n_bins, 
  *   map_dev, kernel_dev  DEVICE npix*npix float32 (any real arrays of the map's shape), not modified
  *   out_dev              DEVICE npix*npix float32, caller-owned; must not alias the inputs
  * The handle keeps the two cuFFT plans and two npix*(npix/2+1) complex spectra between calls (0.8 GB for npix = 10000).
- * MLENS_EINVAL for NULL pointers / bad shape or size; MLENS_ECUDA / MLENS_ENOMEM for CUDA and cuFFT failures. */
+ * MLENS_EINVAL for NULL pointers / bad shape or size; MLENS_ECUDA / MLENS_ENOMEM for CUDA and cuFFT failures.
+ *
+ * mlens_convolve_prepare transforms a kernel ONCE and keeps its spectrum in the handle (another npix*(npix/2+1) complex
+ * numbers); afterwards mlens_convolve may be called with kernel_dev == NULL to reuse it — a survey convolves many maps
+ * with one source profile (~1e6 convolutions), which saves one of the three FFTs per map.  The result is
+ * bit-identical to passing the kernel.  MLENS_EINVAL if kernel_dev is NULL and nothing was prepared. */
 int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kernel_dev, void* cuda_stream);
+int mlens_convolve_prepare(mlens_t* h, const float* kernel_dev, void* cuda_stream);
 int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, float* out_dev, void* cuda_stream);
 
 /* Derived lattice and parameters (pure host data; valid from mlens_create on). */

@@ -80,7 +80,8 @@ struct mlens {
     // convolution (lazily created): cuFFT plans, spectra of the map and of the kernel, profile normalisation scratch
     cufftHandle plan_r2c, plan_c2r;
     int have_plans;
-    float2 *spec_map, *spec_ker;
+    float2 *spec_map, *spec_ker, *spec_prep;  // spectra of the map, of the kernel given to mlens_convolve, of the prepared kernel
+    int have_prep;
     double* prof_sum;
     unsigned long long* idx_hist;      // scratch of mlens_index_map: histogram, LUT, distinct counter
     int* idx_lut;
@@ -399,6 +400,7 @@ void mlens_destroy(mlens_t* h) {
     if (h->have_plans) { cufftDestroy(h->plan_r2c); cufftDestroy(h->plan_c2r); }
     if (h->spec_map) cudaFree(h->spec_map);
     if (h->spec_ker) cudaFree(h->spec_ker);
+    if (h->spec_prep) cudaFree(h->spec_prep);
     if (h->prof_sum) cudaFree(h->prof_sum);
     if (h->counters_host) cudaFreeHost(h->counters_host);
     if (h->count_own) cudaFree(h->count_own);
@@ -673,29 +675,56 @@ int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kerne
             return fail(r_ == CUFFT_ALLOC_FAILED ? MLENS_ENOMEM : MLENS_ECUDA, "%s: cuFFT error %d", #call, (int)r_); \
     } while (0)
 
-int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, float* out_dev, void* cuda_stream) {
-    if (!h || !map_dev || !kernel_dev || !out_dev) return fail(MLENS_EINVAL, "NULL argument");
-    if (int rc = check_handle(h)) return rc;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
+namespace {
+// cuFFT plans (created once per handle) bound to `st`
+int convolve_plans(mlens_t* h, cudaStream_t st) {
     const int N = h->npix;
-    const long long nc = (long long)N * (N / 2 + 1);  // complex elements of an R2C spectrum
     if (!h->have_plans) {
         MLENS_CUFFT(cufftPlan2d(&h->plan_r2c, N, N, CUFFT_R2C));
         cufftResult r = cufftPlan2d(&h->plan_c2r, N, N, CUFFT_C2R);
         if (r != CUFFT_SUCCESS) { cufftDestroy(h->plan_r2c); return fail(MLENS_ECUDA, "cufftPlan2d(C2R): cuFFT error %d", (int)r); }
         h->have_plans = 1;
     }
-    if (!h->spec_map) MLENS_CUDA(cudaMalloc(&h->spec_map, sizeof(float2) * (size_t)nc));
-    if (!h->spec_ker) MLENS_CUDA(cudaMalloc(&h->spec_ker, sizeof(float2) * (size_t)nc));
     MLENS_CUFFT(cufftSetStream(h->plan_r2c, st));
     MLENS_CUFFT(cufftSetStream(h->plan_c2r, st));
+    return MLENS_OK;
+}
+}  // namespace
+
+int mlens_convolve_prepare(mlens_t* h, const float* kernel_dev, void* cuda_stream) {
+    if (!h || !kernel_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long nc = (long long)h->npix * (h->npix / 2 + 1);
+    if (int rc = convolve_plans(h, st)) return rc;
+    if (!h->spec_prep) MLENS_CUDA(cudaMalloc(&h->spec_prep, sizeof(float2) * (size_t)nc));
+    h->have_prep = 0;
+    MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_prep)));
+    h->have_prep = 1;
+    return MLENS_OK;
+}
+
+int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, float* out_dev, void* cuda_stream) {
+    if (!h || !map_dev || !out_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (int rc = check_handle(h)) return rc;
+    if (!kernel_dev && !h->have_prep) return fail(MLENS_EINVAL, "kernel_dev is NULL and no kernel was prepared (mlens_convolve_prepare)");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int N = h->npix;
+    const long long nc = (long long)N * (N / 2 + 1);  // complex elements of an R2C spectrum
+    if (int rc = convolve_plans(h, st)) return rc;
+    if (!h->spec_map) MLENS_CUDA(cudaMalloc(&h->spec_map, sizeof(float2) * (size_t)nc));
     // out-of-place R2C leaves its real input untouched; cuFFT takes non-const pointers
     MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(map_dev), reinterpret_cast<cufftComplex*>(h->spec_map)));
-    MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_ker)));
+    const float2* spec_k = h->spec_prep;  // the prepared spectrum, unless a kernel is given
+    if (kernel_dev) {
+        if (!h->spec_ker) MLENS_CUDA(cudaMalloc(&h->spec_ker, sizeof(float2) * (size_t)nc));
+        MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_ker)));
+        spec_k = h->spec_ker;
+    }
     long long blocks = (nc / 2 + 255) / 256;
     if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
     if (blocks < 1) blocks = 1;
-    mlk::spectral_product_kernel<<<(unsigned)blocks, 256, 0, st>>>(h->spec_map, h->spec_ker, nc, 1.0f / ((float)N * (float)N));
+    mlk::spectral_product_kernel<<<(unsigned)blocks, 256, 0, st>>>(h->spec_map, spec_k, nc, 1.0f / ((float)N * (float)N));
     MLENS_CUDA(cudaGetLastError());
     MLENS_CUFFT(cufftExecC2R(h->plan_c2r, reinterpret_cast<cufftComplex*>(h->spec_map), out_dev));
     return MLENS_OK;

@@ -78,6 +78,7 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_mpd_rebin.argtypes = [vp, vp, ci, ci, dbl, dbl, vp, vp]
     L.mlens_profile_kernel.argtypes = [vp, ci, dbl, vp, vp]
     L.mlens_convolve.argtypes = [vp, vp, vp, vp, vp]
+    L.mlens_convolve_prepare.argtypes = [vp, vp, vp]
     L.mlens_get_geometry.argtypes = [vp, ctypes.POINTER(Geometry)]
     L.mlens_get_stats.argtypes = [vp, vp, ctypes.POINTER(Stats)]
     L.mlens_reset_stats.argtypes = [vp, vp]
@@ -89,7 +90,7 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
                  "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option", "mlens_bits_needed",
-                 "mlens_pack_map", "mlens_unpack_map", "mlens_mpd_rebin"):
+                 "mlens_pack_map", "mlens_unpack_map", "mlens_mpd_rebin", "mlens_convolve_prepare"):
         getattr(L, name).restype = ci
     _libs[key] = L
     return L
@@ -289,17 +290,26 @@ class Mlens:
                                           _stream_ptr(stream)))
         return kernel
 
+    def convolve_prepare(self, kernel, stream=None):
+        """mlens_convolve_prepare: transform a kernel once; later ``convolve(mag, None)`` calls reuse its spectrum."""
+        import torch
+
+        assert kernel.is_cuda and kernel.dtype == torch.float32 and kernel.is_contiguous() and kernel.numel() == self.npix**2
+        self._ck(self._L.mlens_convolve_prepare(self._h, ctypes.c_void_p(kernel.data_ptr()), _stream_ptr(stream)))
+
     def convolve(self, mag, kernel, out=None, stream=None):
-        """mlens_convolve: out = F^-1[F(mag) F(kernel)] (Eq. 6), the circular convolution; float32 [npix,npix]."""
+        """mlens_convolve: out = F^-1[F(mag) F(kernel)] (Eq. 6), the circular convolution; float32 [npix,npix].
+        ``kernel=None`` uses the spectrum kept by ``convolve_prepare``."""
         import torch
 
         if out is None:
             out = torch.empty((self.npix, self.npix), dtype=torch.float32, device="cuda")
         for t in (mag, kernel, out):
-            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.npix**2
-        assert out.data_ptr() not in (mag.data_ptr(), kernel.data_ptr())
-        self._ck(self._L.mlens_convolve(self._h, ctypes.c_void_p(mag.data_ptr()), ctypes.c_void_p(kernel.data_ptr()),
-                                    ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
+            assert t is None or (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() == self.npix**2)
+        assert out.data_ptr() != mag.data_ptr() and (kernel is None or out.data_ptr() != kernel.data_ptr())
+        self._ck(self._L.mlens_convolve(self._h, ctypes.c_void_p(mag.data_ptr()),
+                                        ctypes.c_void_p(kernel.data_ptr()) if kernel is not None else None,
+                                        ctypes.c_void_p(out.data_ptr()), _stream_ptr(stream)))
         return out
 
     def stats(self, stream=None):

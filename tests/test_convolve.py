@@ -111,6 +111,13 @@ def test_profile_kernel_and_convolution_match_the_oracle(oracle, npix, shape, si
         assert np.allclose(Kg, K_ref, rtol=1e-6, atol=0)
         C_gpu = h.convolve(torch.from_numpy(M).cuda(), K_gpu).cpu().numpy().astype(np.float64)
         C_gpu2 = h.convolve(torch.from_numpy(M).cuda(), K_gpu).cpu().numpy()  # plans and spectra are reused
+        with pytest.raises(mlens.MlensError):
+            h.convolve(torch.from_numpy(M).cuda(), None)  # nothing prepared yet
+        h.convolve_prepare(K_gpu)  # the kernel's spectrum kept in the handle: two FFTs per map instead of three
+        C_gpu3 = h.convolve(torch.from_numpy(M).cuda(), None).cpu().numpy()
+        h.convolve(torch.from_numpy(M).cuda(), h.profile_kernel(0, 1.0))  # another kernel in between must not disturb it
+        C_gpu4 = h.convolve(torch.from_numpy(M).cuda(), None).cpu().numpy()
+        assert np.array_equal(C_gpu3, C_gpu2) and np.array_equal(C_gpu4, C_gpu2)
     if npix <= 250:
         C_ref = oracle.convolve(M, Kg)  # same kernel bytes on both sides: this compares the convolution alone
         err = np.abs(C_gpu - C_ref).max()
