@@ -288,6 +288,39 @@ def test_near_list_overflow_falls_back_to_fp64(ml, oracle):
             assert r["l1"] <= max(2, 2 * r["mismatch"]) and r["mismatch"] <= 2
 
 
+@pytest.mark.parametrize("case", range(12))
+def test_seeded_random_small_maps_against_the_oracle(ml, oracle, case):
+    # whole small maps with seeded random parameters: both parities of both macro factors (kappa + gamma > 1: saddle /
+    # over-focused images), negative shear, all-smooth and no-smooth matter, unit and Salpeter masses, maps narrower than
+    # one tile, lens counts from 0 to a few hundred
+    u = fields.uniform01(9000 + case, 0, 16)
+    kappa = [0.2, 0.45, 0.7, 1.3, 1.6, 0.9][case % 6] + 0.05 * u[0]
+    gamma = (0.6 * u[1] - 0.3) if case % 3 else (0.5 + 0.4 * u[1])
+    if abs(1 - kappa - gamma) < 0.05 or abs(1 - kappa + gamma) < 0.05:
+        gamma += 0.11
+    s = [0.0, 0.3, 1.0, 0.8][case % 4]
+    npix = [24, 40, 64, 17][case % 4]
+    sub = [3, 2, 4, 5][(case // 2) % 4]
+    L = [2.0, 6.0, 1.0][case % 3]
+    n_lens = 0 if s == 1.0 else [3, 40, 150, 12][case % 4]
+    masses = "salpeter" if case % 2 else "unit"
+    cfg = fields.MapConfig(f"rnd{case}", npix, L, kappa, gamma, s, sub, masses, 9100 + case)
+    xy, m = fields.random_field(n_lens, max(cfg.disc_radius, 1.0), 9100 + case, masses)
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        count, mag, st = h.shoot()
+        c = count.cpu().numpy().astype(np.int64)
+        g = h.geometry
+    ref = oracle.shoot_block(*_args(cfg), xy, m)
+    rs = ref["stats"]
+    l1 = int(np.abs(c - ref["count"]).sum())
+    assert (g.n1, g.n2) == (ref["geometry"].n1, ref["geometry"].n2)
+    assert st["rays_total"] == rs["rays_total"] == g.n1 * g.n2 and st["rays_lost"] == rs["rays_lost"]
+    assert st["rays_in_map"] + st["rays_outside"] + st["rays_lost"] == st["rays_total"]
+    assert l1 <= max(2, TOL_L1 * rs["rays_in_map"]), (case, kappa, gamma, s, l1, rs)
+    assert abs(st["rays_in_map"] - rs["rays_in_map"]) <= l1
+    assert np.array_equal(mag.cpu().numpy(), oracle.magnification(c.astype(np.int32), g.n_avg))
+
+
 def test_mirror_symmetry_on_gpu(ml):
     # P6 through the CUDA path
     cfg = dataclasses.replace(fields.CONFIGS[1], npix=128, sub=6)
