@@ -10,7 +10,7 @@ another.  One JSON line is printed by rank 0.
 
 * `value`      ray-lens interactions/s, all ranks, device-timed (CUDA events on the launching stream), max over ranks.
 * `e2e`        the same metric through `mlens_create` + `mlens_shoot_host` + `mlens_destroy` with HOST buffers (lens
-               arrays in, count + magnification maps out), copies inside the timed region.
+               arrays in, count + magnification maps out into pinned host memory), copies inside the timed region.
 * `roofline`   the shooting kernel alone: 11 flops x interactions / kernel time (events inside libmlens around the
                kernel launch) against the FP32 peak SMs x 128 x 2 x f_max; bound = "alu".
                `peak_measured` / `frac_of_measured`: the scalar-FFMA rate measured on this box just before the timed
@@ -338,15 +338,25 @@ def run_ours(args):
     h.close()
     barrier()
     e2e_kernel_ms = []
+    # the caller's result buffers: pinned host memory, allocated once and reused for every map (as a survey would)
+    c_pin = torch.empty((cfg.npix, cfg.npix), dtype=torch.int32, pin_memory=True)
+    m_pin = torch.empty((cfg.npix, cfg.npix), dtype=torch.float32, pin_memory=True)
+    e2e_phase_ms = []  # host clock per step: [mlens_create (H2D of the lens list), shoot + D2H, mlens_destroy]
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        with mlens.Mlens.from_config(cfg, xy, m) as h2:
-            if shard:
-                c_dev, m_dev, st2 = sharded.shoot_sharded(h2, rank, world)
-                c_host, m_host = c_dev.cpu().numpy(), m_dev.cpu().numpy()
-            else:
-                c_host, m_host, st2 = h2.shoot_host()
-            e2e_kernel_ms.append(st2.get("kernel_ms"))
+        ta = time.perf_counter()
+        h2 = mlens.Mlens.from_config(cfg, xy, m)
+        tb = time.perf_counter()
+        if shard:
+            c_dev, m_dev, st2 = sharded.shoot_sharded(h2, rank, world)
+            c_host, m_host = c_dev.cpu().numpy(), m_dev.cpu().numpy()
+        else:
+            c_host, m_host, st2 = h2.shoot_host(count=c_pin.numpy(), mag=m_pin.numpy())
+        tc = time.perf_counter()
+        h2.close()
+        td = time.perf_counter()
+        e2e_kernel_ms.append(st2.get("kernel_ms"))
+        e2e_phase_ms.append([round(1e3 * (tb - ta), 3), round(1e3 * (tc - tb), 3), round(1e3 * (td - tc), 3)])
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
@@ -364,6 +374,7 @@ def run_ours(args):
                          h2d_bytes=xy.nbytes + m.nbytes, d2h_bytes=c_host.nbytes + m_host.nbytes, peak_meas=peak_meas,
                          traffic=traffic, traffic_source=traffic_source)
         line["e2e"]["kernel_ms_per_step"] = e2e_kernel_ms  # of which: the shooting kernel (events inside libmlens)
+        line["e2e"]["host_ms_per_step_create_shoot_destroy"] = e2e_phase_ms
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = run_cpu_baseline(cfg, xy, m)
         print(json.dumps(line), flush=True)

@@ -189,13 +189,18 @@ class Mlens:
                                        ctypes.c_void_p(pix.data_ptr()) if pix is not None else None, _stream_ptr(stream)))
         return {"count": count, "y": y, "pix": pix}
 
-    def shoot_host(self, want_mag=True):
-        """mlens_shoot_host: HOST numpy buffers in and out (the end-to-end call)."""
-        count = np.empty((self.npix, self.npix), dtype=np.int32)
-        mag = np.empty((self.npix, self.npix), dtype=np.float32) if want_mag else None
+    def shoot_host(self, want_mag=True, count=None, mag=None):
+        """mlens_shoot_host: HOST numpy buffers in and out (the end-to-end call).  ``count`` / ``mag`` may be caller-owned
+        C-contiguous int32 / float32 arrays of npix*npix elements (e.g. views of pinned memory, reused between maps)."""
+        if count is None:
+            count = np.empty((self.npix, self.npix), dtype=np.int32)
+        if mag is None and want_mag:
+            mag = np.empty((self.npix, self.npix), dtype=np.float32)
+        assert count.dtype == np.int32 and count.flags.c_contiguous and count.size == self.npix**2
+        assert mag is None or (mag.dtype == np.float32 and mag.flags.c_contiguous and mag.size == self.npix**2)
         st = Stats()
         self._ck(self._L.mlens_shoot_host(self._h, count.ctypes.data_as(ctypes.c_void_p),
-                                      mag.ctypes.data_as(ctypes.c_void_p) if mag is not None else None, ctypes.byref(st)))
+                                          mag.ctypes.data_as(ctypes.c_void_p) if mag is not None else None, ctypes.byref(st)))
         return count, mag, st.as_dict()
 
     def magnification(self, count, mag=None, stream=None):

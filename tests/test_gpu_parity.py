@@ -132,6 +132,10 @@ def test_tiny_config_full_map(ml, oracle):
         assert (h.geometry.n1, h.geometry.n2) == (6144, 3414)
         count, mag, st = h.shoot()
         host_count, host_mag, host_st = h.shoot_host()
+        pin_c = torch.empty((cfg.npix, cfg.npix), dtype=torch.int32, pin_memory=True)
+        pin_m = torch.empty((cfg.npix, cfg.npix), dtype=torch.float32, pin_memory=True)
+        h.shoot_host(count=pin_c.numpy(), mag=pin_m.numpy())  # caller-owned (pinned) result buffers
+        assert np.array_equal(pin_c.numpy(), host_count) and np.array_equal(pin_m.numpy(), host_mag)
     ref = oracle.shoot_block(*_args(cfg), xy, m)
     c = count.cpu().numpy()
     l1 = int(np.abs(c.astype(np.int64) - ref["count"]).sum())
