@@ -461,6 +461,20 @@ def run_mpd(args):
             torch.cuda.synchronize()
             dms.append(e0.elapsed_time(e1))
         assert torch.equal(back, count)
+        # minimal-bit-width storage: the indexed map at the width of its largest index, and back
+        bits = int(mlens.lib().mlens_bits_needed(int(values.numel()) - 1))
+        pms, ums = [], []
+        for _ in range(args.steps):
+            flush.fill_(1)
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0.record()
+            packed = h.pack_map(indexed, bits)
+            e1.record()
+            unpacked = h.unpack_map(packed, bits, dtype=torch.uint16)
+            e2.record()
+            torch.cuda.synchronize()
+            pms.append(e0.elapsed_time(e1)); ums.append(e1.elapsed_time(e2))
+        assert torch.equal(unpacked, indexed)
     med = statistics.median(ms)
     nbytes = 4 * cfg.npix**2
     peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(
@@ -473,7 +487,12 @@ def run_mpd(args):
                       "index_map": {"n_distinct": int(values.numel()), "ms_median_host_clock": statistics.median(ims),
                                     "unindex_ms_median": statistics.median(dms),
                                     "algorithmic_bytes": 10 * cfg.npix**2,  # MPD pass 4 B + apply 4 B in + 2 B out per pixel
-                                    "unindex_gbs": 6 * cfg.npix**2 / (statistics.median(dms) * 1e-3) / 1e9}}), flush=True)
+                                    "unindex_gbs": 6 * cfg.npix**2 / (statistics.median(dms) * 1e-3) / 1e9},
+                      "pack_indexed_map": {"bits": bits, "pack_ms_median": statistics.median(pms), "unpack_ms_median": statistics.median(ums),
+                                           "algorithmic_bytes": (2 + bits / 8) * cfg.npix**2,
+                                           "pack_gbs": (2 + bits / 8) * cfg.npix**2 / (statistics.median(pms) * 1e-3) / 1e9,
+                                           "unpack_gbs": (2 + bits / 8) * cfg.npix**2 / (statistics.median(ums) * 1e-3) / 1e9}}),
+          flush=True)
 
 
 def run_convolve(args):
