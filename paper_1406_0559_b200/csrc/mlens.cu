@@ -235,7 +235,8 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         const double zmax = (h->lens_extent + std::fmax(h->geo.a1, h->geo.a2)) / h->d;  // per axis, lattice units
         if (shared > 0 && 4.0 * zmax * zmax * zmax * zmax > 1.0e37) shared = 0;
         const int code = h->opt_rays * 10000 + h->opt_tile_x * 10 + shared;
-        const bool runs = h->opt_binning == mlk::BIN_RUNS;  // the default binning route is compiled in (shorter epilogue)
+        // the default launch (run-combining REDs into a count map, no per-ray outputs) has its own, leaner instantiation
+        const bool runs = h->opt_binning == mlk::BIN_RUNS && count != nullptr && ray_y == nullptr && ray_pix == nullptr;
         switch (code) {
 #define MLENS_VARIANT(TX, R, SP, NC)                                                                                       \
     case R * 10000 + TX * 10 + SP:                                                                                          \

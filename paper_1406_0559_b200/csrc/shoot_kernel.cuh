@@ -423,7 +423,10 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
         const long long jray = tj0 + ty;
         const bool row_ok = jray < P.j0 + P.nj;
         const double x2 = ((double)jray + 0.5 - P.half_n2) * P.d;
-        int n_in = 0, n_out = 0, n_lost = 0;
+        // rays k < k_valid of this thread lie inside the shot block (ragged right / bottom edge of the block)
+        const long long k_room = P.i0 + P.ni - (ti0 + (long long)tx * kR);
+        const int k_valid = row_ok ? (int)(k_room < 0 ? 0 : (k_room > kR ? kR : k_room)) : 0;
+        int n_in = 0, n_lost = 0;
         int run_pix = -1, run_n = 0;
 
         if (bin_mode == BIN_WINDOW) {
@@ -448,8 +451,10 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
         const double U2c = (P.f2 * Zcy + Aci + P.half_L) * P.inv_p;
         const double dyt = ((double)ty - 31.5) * P.d;        // exact in-tile offsets in R_E
         const bool special = n_near > 0 || near_overflow;    // tile-uniform: near-lens list or FP64 fallback in play
-        const bool want_rays = P.ray_y != nullptr || P.ray_pix != nullptr;
-        const double npix_d = (double)P.npix;
+        // the production instantiation (kBin >= 0) is only launched with a count map and without per-ray outputs
+        const bool want_rays = kBin < 0 && (P.ray_y != nullptr || P.ray_pix != nullptr);
+        const bool have_count = kBin >= 0 || P.count != nullptr;
+        const unsigned npix_u = (unsigned)P.npix;
         const double dip = P.d * P.inv_p;                     // lattice step in pixels
         // u1 of ray k = B1 + k*s1 + (delta*S)_re * d/p  with the thread's first in-tile offset folded into B1
         const double s1 = P.f1 * dip;
@@ -462,8 +467,7 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
             const float eps = (float)k - 0.5f * (float)(kR - 1);
             const float srf = sre[k], sif = sim[k];
             const float dxf = cxf + eps;                     // in-tile offset in lattice steps (exact)
-            const long long iray = ti0 + tx * kR + k;
-            const bool ok = row_ok && iray < P.i0 + P.ni;
+            const bool ok = k < k_valid;
             // conj(alpha) = A_c - delta*S ; alpha = (Re, -Im);  y1 = f1 x1 - alpha1,  y2 = f2 x2 - alpha2
             const float ds_re = dxf * srf - dyf * sif;       // (delta * S) / d
             const float ds_im = dxf * sif + dyf * srf;
@@ -472,29 +476,29 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
             bool finite = fabsf(ds_re) <= 3.4028234663852886e38f && fabsf(ds_im) <= 3.4028234663852886e38f;
             if (special) {
                 // exact FP64 in-tile offsets here: a ray 1e-4 R_E from a lens sees a deflection gradient m/r^2 ~ 1e8
+                const long long iray = ti0 + tx * kR + k;
                 const double2 u = special_ray(P, sh, n_near, near_overflow, Acr - (double)ds_re * P.d, -(Aci - (double)ds_im * P.d),
                                               (dxt0 + (double)k) * P.d, dyt, ((double)iray + 0.5 - P.half_n1) * P.d, x2);
                 u1 = u.x; u2 = u.y;
                 finite = fabs(u1) <= 1.7976931348623157e308 && fabs(u2) <= 1.7976931348623157e308;
             }
-            int pix;
-            if (!finite) {
-                pix = -2;  // non-finite source position (ray on a lens): lost
-            } else if (u1 >= 0.0 && u1 < npix_d && u2 >= 0.0 && u2 < npix_d) {
-                pix = floor_to_int(u2) * P.npix + floor_to_int(u1);
-            } else {
-                pix = -1;
+            // Pixel of u: t = u + 1.5 * 2^52 rounded DOWN is 1.5 * 2^52 + floor(u) exactly while |u| < 2^51, so its high
+            // word is 0x43380000 iff 0 <= floor(u) < 2^32 and its low word is floor(u): "0 <= u < npix" and the floor in
+            // one FP64 add and two integer compares per coordinate (anything else — negative, huge, inf, NaN — fails the
+            // high-word test).
+            const double t1 = __dadd_rd(u1, 6755399441055744.0), t2 = __dadd_rd(u2, 6755399441055744.0);
+            const unsigned ix = (unsigned)__double2loint(t1), iy = (unsigned)__double2loint(t2);
+            const bool in = finite && __double2hiint(t1) == 0x43380000 && __double2hiint(t2) == 0x43380000 && ix < npix_u && iy < npix_u;
+            const int pix = in ? (int)(iy * npix_u + ix) : (finite ? -1 : -2);  // -2: non-finite source position (lost)
+            n_in += (ok && in);
+            if (!finite && ok) ++n_lost;
+            if (want_rays && ok) {
+                const long long qidx = (jray - P.j0) * P.ni + (ti0 + tx * kR + k - P.i0);
+                if (P.ray_y) { P.ray_y[2 * qidx] = u1 * P.p - P.half_L; P.ray_y[2 * qidx + 1] = u2 * P.p - P.half_L; }
+                if (P.ray_pix) P.ray_pix[qidx] = pix;
             }
-            if (ok) {
-                n_in += (pix >= 0); n_out += (pix == -1); n_lost += (pix == -2);
-                if (want_rays) {
-                    const long long qidx = (jray - P.j0) * P.ni + (iray - P.i0);
-                    if (P.ray_y) { P.ray_y[2 * qidx] = u1 * P.p - P.half_L; P.ray_y[2 * qidx + 1] = u2 * P.p - P.half_L; }
-                    if (P.ray_pix) P.ray_pix[qidx] = pix;
-                }
-            }
-            if (P.count) {
-                const int bp = ok ? pix : -1;
+            if (have_count) {
+                const int bp = (ok && in) ? pix : -1;
                 if (bin_mode == BIN_PER_RAY) {
                     if (bp >= 0) red_add(P.count + bp, 1);
                 } else {
@@ -505,7 +509,8 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
                 }
             }
         }
-        if (P.count && bin_mode != BIN_PER_RAY) flush_run(P, sh, bin_mode, run_pix, run_n, run_pix >= 0);
+        if (have_count && bin_mode != BIN_PER_RAY) flush_run(P, sh, bin_mode, run_pix, run_n, run_pix >= 0);
+        int n_out = k_valid - n_in - n_lost;  // finite, outside the map
         n_in = __reduce_add_sync(0xffffffffu, n_in);
         n_out = __reduce_add_sync(0xffffffffu, n_out);
         n_lost = __reduce_add_sync(0xffffffffu, n_lost);
@@ -515,7 +520,7 @@ __global__ void __launch_bounds__(kTX / kR * kTile, kMinCtas) shoot_fp32_kernel(
             if (n_lost) atomicAdd(&sh.ctr[2], (unsigned long long)n_lost);
         }
         __syncthreads();  // all epilogues done: near list and window are complete
-        if (bin_mode == BIN_WINDOW && P.count) {
+        if (bin_mode == BIN_WINDOW && have_count) {
             for (int t = tid; t < kWin * kWin; t += kThreads) {
                 const int v = sh.win[t];
                 if (v) {
