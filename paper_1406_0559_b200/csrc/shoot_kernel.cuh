@@ -27,7 +27,7 @@
 #include <stdint.h>
 
 #ifndef MLENS_HOT_UNROLL
-#define MLENS_HOT_UNROLL 24  // lenses per unrolled hot-loop iteration; re-swept after every change of the surrounding code
+#define MLENS_HOT_UNROLL 28  // lenses per unrolled hot-loop iteration; re-swept after every change of the surrounding code
 #endif
 
 namespace mlk {
