@@ -235,8 +235,14 @@ int mlens_set_option(mlens_t* h, const char* key, long long value);
 /* Thread-local message for the last failure on this thread ("" if none). */
 const char* mlens_last_error(void);
 
-/* Frees everything mlens_create allocated (never the caller's buffers).  NULL is allowed. */
+/* Frees everything mlens_create allocated (never the caller's buffers), after synchronising the handle's device.  NULL
+ * is allowed.  Device blocks return to a library-owned memory pool (one per device) that KEEPS them for the next
+ * handle, so that creating / shooting / destroying map after map does not pay cudaMalloc / cudaFree each time (cudaFree
+ * of a map-sized buffer was measured at up to 1.5 s on the B200 box). */
 void mlens_destroy(mlens_t* h);
+
+/* Hand the blocks cached by destroyed handles on the CURRENT device back to the driver (blocks of live handles stay). */
+int mlens_trim_memory(void);
 
 #ifdef __cplusplus
 }

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -42,6 +43,79 @@ int fail(int code, const char* fmt, ...) {
                         cudaGetErrorString(e_));                                                      \
     } while (0)
 
+// Device memory of the handles comes from ONE library-owned stream-ordered pool per device that keeps freed blocks
+// (release threshold = max): mlens_create / mlens_shoot_host / mlens_destroy of map after map then recycle the same
+// blocks.  Measured on the B200 box: cudaFree of the 64 MB result buffers took 20 ... 1500 ms on one call in three, i.e.
+// up to 1.6x the whole 0.88 s map of config 3 (profiles/r2_summary.md, "e2e"); cudaFreeAsync into the pool returns at once.
+// mlens_trim_memory() hands the cached blocks back to the driver.
+struct DevPool {
+    cudaMemPool_t pool = nullptr;
+    cudaStream_t stream = nullptr;
+    int state = 0;  // 0 = not tried, 1 = pool in use, -1 = unavailable: plain cudaMalloc / cudaFree
+};
+std::mutex g_pool_mutex;
+DevPool g_pools[64];
+
+DevPool* device_pool() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    DevPool* dp = &g_pools[dev];
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (dp->state == 0) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        unsigned long long keep = ~0ull;
+        if (cudaMemPoolCreate(&dp->pool, &props) == cudaSuccess &&
+            cudaMemPoolSetAttribute(dp->pool, cudaMemPoolAttrReleaseThreshold, &keep) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&dp->stream, cudaStreamNonBlocking) == cudaSuccess) {
+            dp->state = 1;
+        } else {
+            (void)cudaGetLastError();
+            dp->state = -1;
+        }
+    }
+    return dp->state == 1 ? dp : nullptr;
+}
+
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t bytes) {
+    if (DevPool* dp = device_pool()) {
+        cudaError_t e = cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes, dp->pool, dp->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(dp->stream);  // usable from any stream from here on
+        return e;
+    }
+    return cudaMalloc(reinterpret_cast<void**>(p), bytes);
+}
+
+// The caller has made sure that no work still uses the block (mlens_destroy synchronises the device first).
+void dev_free(void* p) {
+    if (!p) return;
+    if (DevPool* dp = device_pool()) cudaFreeAsync(p, dp->stream);
+    else cudaFree(p);
+}
+
+// The handles' small pinned host mirrors (64-byte blocks) are recycled the same way: cudaMallocHost costs 2-10 ms.
+constexpr size_t kPinnedBlock = 64;
+std::vector<void*> g_pinned_free;
+
+cudaError_t pinned_alloc(void** p) {
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mutex);
+        if (!g_pinned_free.empty()) { *p = g_pinned_free.back(); g_pinned_free.pop_back(); return cudaSuccess; }
+    }
+    return cudaMallocHost(p, kPinnedBlock);
+}
+
+void pinned_free(void* p) {
+    if (!p) return;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    try { g_pinned_free.push_back(p); } catch (...) { cudaFreeHost(p); }
+}
+
 constexpr int kChunkMax = 2048;        // lenses per chunk when the list is streamed in several chunks
 constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chunk
 // The production instantiation of shoot_fp32_kernel (chosen by the sweep in profiles/): tile width,
@@ -60,6 +134,8 @@ constexpr int kProdCtas = 2;
 constexpr int kTileCtrSlots = 256;     // ring of dynamic tile counters: one per launch in flight (see launch_block)
 
 }  // namespace
+
+static_assert(sizeof(mlk::MapStatsDev) <= kPinnedBlock && 8 * sizeof(unsigned long long) <= kPinnedBlock, "pinned mirror block");
 
 struct mlens {
     // parameters
@@ -173,7 +249,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
                     for (int k = 0; k < 8; ++k)
                         A[((size_t)rb * mlk::kUmABlockBytes + mlk::umma_off_bytes(r, k)) / 4] = row[k];
                 }
-            MLENS_CUDA(cudaMalloc(&h->umma_A_dev, A.size() * sizeof(float)));
+            MLENS_CUDA(dev_alloc(&h->umma_A_dev, A.size() * sizeof(float)));
             MLENS_CUDA(cudaMemcpy(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice));
         }
         P.umma_A = h->umma_A_dev;
@@ -347,31 +423,36 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
 
     int dev = 0;
     MLENS_CUDA(cudaGetDevice(&dev));
-    cudaDeviceProp prop;
-    MLENS_CUDA(cudaGetDeviceProperties(&prop, dev));
-    if (prop.major != 10) return fail(MLENS_ECUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
+    // three attributes, not cudaGetDeviceProperties: that call alone costs milliseconds, more than config 1's whole map
+    int cc_major = 0, cc_minor = 0, sm_count = 0;
+    MLENS_CUDA(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    MLENS_CUDA(cudaDeviceGetAttribute(&cc_minor, cudaDevAttrComputeCapabilityMinor, dev));
+    MLENS_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+    if (cc_major != 10) return fail(MLENS_ECUDA, "device %d is sm_%d%d; this library is built for sm_100a only", dev, cc_major, cc_minor);
 
     mlens* h = new (std::nothrow) mlens();
     if (!h) return fail(MLENS_ENOMEM, "host allocation failed");
     memset(h, 0, sizeof(*h));
     h->kappa = kappa; h->gamma = gamma; h->s = s; h->L = map_side; h->d = ray_spacing;
     h->npix = npix; h->n_lens = n_lens; h->geo = g;
-    h->device = dev; h->sm_count = prop.multiProcessorCount;
+    h->device = dev; h->sm_count = sm_count;
     h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 0; h->opt_shared = 0; h->opt_rays = kProdRays;
     h->opt_tile_x = kProdTileX; h->opt_shared_pairs = kProdSharedPairs;
     for (long long k = 0; k < n_lens; ++k)
         h->lens_extent = std::fmax(h->lens_extent, std::fmax(std::fabs((double)packed[(size_t)k].x), std::fabs((double)packed[(size_t)k].y)));
 
     cudaError_t e = cudaSuccess;
-    if (e == cudaSuccess) e = cudaMalloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
+    if (e == cudaSuccess) e = dev_alloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
     if (e == cudaSuccess && n_lens > 0)
         e = cudaMemcpy(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(&h->counters_dev, 8 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, 8 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMalloc(&h->tile_ctr_dev, kTileCtrSlots * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMalloc(&h->max_count_dev, sizeof(int));
-    if (e == cudaSuccess) e = cudaMemset(h->max_count_dev, 0, sizeof(int));
-    if (e == cudaSuccess) e = cudaMallocHost(&h->counters_host, 8 * sizeof(unsigned long long));
+    // one block for the small device state: 8 ray counters, the ring of tile counters, max_count
+    if (e == cudaSuccess) e = dev_alloc(&h->counters_dev, (8 + kTileCtrSlots + 1) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, (8 + kTileCtrSlots + 1) * sizeof(unsigned long long));
+    if (e == cudaSuccess) {
+        h->tile_ctr_dev = h->counters_dev + 8;
+        h->max_count_dev = reinterpret_cast<int*>(h->counters_dev + 8 + kTileCtrSlots);
+    }
+    if (e == cudaSuccess) e = pinned_alloc(reinterpret_cast<void**>(&h->counters_host));
     if (e == cudaSuccess) e = cudaEventCreate(&h->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&h->ev1);
     if (e == cudaSuccess) e = cudaEventCreate(&h->evk0);
@@ -387,31 +468,44 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
 
 void mlens_destroy(mlens_t* h) {
     if (!h) return;
-    if (h->lens_dev) cudaFree(h->lens_dev);
-    if (h->counters_dev) cudaFree(h->counters_dev);
-    if (h->tile_ctr_dev) cudaFree(h->tile_ctr_dev);
-    if (h->max_count_dev) cudaFree(h->max_count_dev);
-    if (h->mapstats_dev) cudaFree(h->mapstats_dev);
-    if (h->mapstats_host) cudaFreeHost(h->mapstats_host);
-    if (h->mpd_partial) cudaFree(h->mpd_partial);
-    if (h->umma_A_dev) cudaFree(h->umma_A_dev);
-    if (h->idx_hist) cudaFree(h->idx_hist);
-    if (h->idx_lut) cudaFree(h->idx_lut);
-    if (h->idx_n_dev) cudaFree(h->idx_n_dev);
+    // the handle's blocks go back to ITS device's pool: make that device current for the duration, and let every kernel
+    // that may still use them finish first (what cudaFree used to do implicitly)
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != h->device) cudaSetDevice(h->device);
+    cudaDeviceSynchronize();
+    dev_free(h->lens_dev);
+    dev_free(h->counters_dev);  // also holds the tile counters and max_count
+    dev_free(h->mapstats_dev);
+    pinned_free(h->mapstats_host);
+    dev_free(h->mpd_partial);
+    dev_free(h->umma_A_dev);
+    dev_free(h->idx_hist);
+    dev_free(h->idx_lut);
+    dev_free(h->idx_n_dev);
     if (h->have_plans) { cufftDestroy(h->plan_r2c); cufftDestroy(h->plan_c2r); }
-    if (h->spec_map) cudaFree(h->spec_map);
-    if (h->spec_ker) cudaFree(h->spec_ker);
-    if (h->spec_prep) cudaFree(h->spec_prep);
-    if (h->prof_sum) cudaFree(h->prof_sum);
-    if (h->counters_host) cudaFreeHost(h->counters_host);
-    if (h->count_own) cudaFree(h->count_own);
-    if (h->mag_own) cudaFree(h->mag_own);
+    dev_free(h->spec_map);
+    dev_free(h->spec_ker);
+    dev_free(h->spec_prep);
+    dev_free(h->prof_sum);
+    pinned_free(h->counters_host);
+    dev_free(h->count_own);
+    dev_free(h->mag_own);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     if (h->evk0) cudaEventDestroy(h->evk0);
     if (h->evk1) cudaEventDestroy(h->evk1);
+    if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
     delete h;
+}
+
+int mlens_trim_memory(void) {
+    if (DevPool* dp = device_pool()) {
+        MLENS_CUDA(cudaStreamSynchronize(dp->stream));
+        MLENS_CUDA(cudaMemPoolTrimTo(dp->pool, 0));
+    }
+    return MLENS_OK;
 }
 
 int mlens_get_geometry(const mlens_t* h, mlens_geometry* g) {
@@ -490,13 +584,13 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
     if (int rc = check_handle(h)) return rc;
     if (n_bins < 2) return fail(MLENS_EINVAL, "n_bins must be >= 2");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (!h->mapstats_dev) MLENS_CUDA(cudaMalloc(&h->mapstats_dev, sizeof(mlk::MapStatsDev)));
-    if (!h->mapstats_host) MLENS_CUDA(cudaMallocHost(&h->mapstats_host, sizeof(mlk::MapStatsDev)));
+    if (!h->mapstats_dev) MLENS_CUDA(dev_alloc(&h->mapstats_dev, sizeof(mlk::MapStatsDev)));
+    if (!h->mapstats_host) MLENS_CUDA(pinned_alloc(reinterpret_cast<void**>(&h->mapstats_host)));
     const long long n = (long long)h->npix * h->npix;
     MLENS_CUDA(cudaMemsetAsync(h->mapstats_dev, 0, sizeof(mlk::MapStatsDev), st));
     MLENS_CUDA(cudaMemsetAsync(hist_dev, 0, sizeof(unsigned long long) * (size_t)n_bins, st));
     if (!h->mpd_partial)
-        MLENS_CUDA(cudaMalloc(&h->mpd_partial, sizeof(unsigned int) * (size_t)h->sm_count * mlk::kMpdSmemBinsMax));
+        MLENS_CUDA(dev_alloc(&h->mpd_partial, sizeof(unsigned int) * (size_t)h->sm_count * mlk::kMpdSmemBinsMax));
     // shared-memory bins: all of them when they fit (multiple of 1024 for the fill/flush loops), else the first 48 Ki
     int smem_bins = (n_bins + 1023) & ~1023;
     if (smem_bins > mlk::kMpdSmemBinsMax) smem_bins = mlk::kMpdSmemBinsMax;
@@ -540,14 +634,14 @@ int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_v
     const long long n_bins = (long long)max_count + 2;
     if (n_bins > 2147483647LL) return fail(MLENS_ERANGE, "largest count %d: the histogram would need more than 2^31-1 bins", max_count);
     if (n_bins > h->idx_bins_cap) {
-        if (h->idx_hist) cudaFree(h->idx_hist);
-        if (h->idx_lut) cudaFree(h->idx_lut);
+        dev_free(h->idx_hist);
+        dev_free(h->idx_lut);
         h->idx_hist = nullptr; h->idx_lut = nullptr; h->idx_bins_cap = 0;
-        MLENS_CUDA(cudaMalloc(&h->idx_hist, sizeof(unsigned long long) * (size_t)n_bins));
-        MLENS_CUDA(cudaMalloc(&h->idx_lut, sizeof(int) * (size_t)n_bins));
+        MLENS_CUDA(dev_alloc(&h->idx_hist, sizeof(unsigned long long) * (size_t)n_bins));
+        MLENS_CUDA(dev_alloc(&h->idx_lut, sizeof(int) * (size_t)n_bins));
         h->idx_bins_cap = n_bins;
     }
-    if (!h->idx_n_dev) MLENS_CUDA(cudaMalloc(&h->idx_n_dev, sizeof(int)));
+    if (!h->idx_n_dev) MLENS_CUDA(dev_alloc(&h->idx_n_dev, sizeof(int)));
     // (2) the MPD histogram: its non-empty bins are the distinct ray-count values
     if (int rc = mlens_mpd(h, count_dev, h->idx_hist, (int)n_bins, cuda_stream, nullptr)) return rc;
     // (3) compaction -> index file (values, ascending) and the count -> index table
@@ -654,7 +748,7 @@ int mlens_profile_kernel(mlens_t* h, int shape, double size_pixels, float* kerne
     if (2.0 * half + 1.0 > (double)h->npix) return fail(MLENS_EINVAL, "profile support (%g pixels) does not fit the %d-pixel map", 2.0 * half + 1.0, h->npix);
     const int R = (int)half;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (!h->prof_sum) MLENS_CUDA(cudaMalloc(&h->prof_sum, sizeof(double)));
+    if (!h->prof_sum) MLENS_CUDA(dev_alloc(&h->prof_sum, sizeof(double)));
     MLENS_CUDA(cudaMemsetAsync(h->prof_sum, 0, sizeof(double), st));
     const long long ns = (2LL * R + 1) * (2LL * R + 1);
     long long b1 = (ns + 255) / 256;
@@ -698,7 +792,7 @@ int mlens_convolve_prepare(mlens_t* h, const float* kernel_dev, void* cuda_strea
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long nc = (long long)h->npix * (h->npix / 2 + 1);
     if (int rc = convolve_plans(h, st)) return rc;
-    if (!h->spec_prep) MLENS_CUDA(cudaMalloc(&h->spec_prep, sizeof(float2) * (size_t)nc));
+    if (!h->spec_prep) MLENS_CUDA(dev_alloc(&h->spec_prep, sizeof(float2) * (size_t)nc));
     h->have_prep = 0;
     MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_prep)));
     h->have_prep = 1;
@@ -713,12 +807,12 @@ int mlens_convolve(mlens_t* h, const float* map_dev, const float* kernel_dev, fl
     const int N = h->npix;
     const long long nc = (long long)N * (N / 2 + 1);  // complex elements of an R2C spectrum
     if (int rc = convolve_plans(h, st)) return rc;
-    if (!h->spec_map) MLENS_CUDA(cudaMalloc(&h->spec_map, sizeof(float2) * (size_t)nc));
+    if (!h->spec_map) MLENS_CUDA(dev_alloc(&h->spec_map, sizeof(float2) * (size_t)nc));
     // out-of-place R2C leaves its real input untouched; cuFFT takes non-const pointers
     MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(map_dev), reinterpret_cast<cufftComplex*>(h->spec_map)));
     const float2* spec_k = h->spec_prep;  // the prepared spectrum, unless a kernel is given
     if (kernel_dev) {
-        if (!h->spec_ker) MLENS_CUDA(cudaMalloc(&h->spec_ker, sizeof(float2) * (size_t)nc));
+        if (!h->spec_ker) MLENS_CUDA(dev_alloc(&h->spec_ker, sizeof(float2) * (size_t)nc));
         MLENS_CUFFT(cufftExecR2C(h->plan_r2c, const_cast<float*>(kernel_dev), reinterpret_cast<cufftComplex*>(h->spec_ker)));
         spec_k = h->spec_ker;
     }
@@ -758,8 +852,8 @@ int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* 
     if (int rc = check_handle(h)) return rc;
     const size_t n = (size_t)h->npix * h->npix;
     if (!h->own_stream) MLENS_CUDA(cudaStreamCreateWithFlags(&h->own_stream, cudaStreamNonBlocking));
-    if (!h->count_own) MLENS_CUDA(cudaMalloc(&h->count_own, n * sizeof(int)));
-    if (mag_host && !h->mag_own) MLENS_CUDA(cudaMalloc(&h->mag_own, n * sizeof(float)));
+    if (!h->count_own) MLENS_CUDA(dev_alloc(&h->count_own, n * sizeof(int)));
+    if (mag_host && !h->mag_own) MLENS_CUDA(dev_alloc(&h->mag_own, n * sizeof(float)));
     mlens_stats local;
     if (int rc = mlens_shoot(h, h->count_own, mag_host ? h->mag_own : nullptr, h->own_stream, &local)) return rc;
     MLENS_CUDA(cudaMemcpyAsync(count_host, h->count_own, n * sizeof(int), cudaMemcpyDeviceToHost, h->own_stream));

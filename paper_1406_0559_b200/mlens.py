@@ -85,6 +85,8 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_set_option.argtypes = [vp, ctypes.c_char_p, ll]
     L.mlens_last_error.argtypes = []
     L.mlens_last_error.restype = ctypes.c_char_p
+    L.mlens_trim_memory.argtypes = []
+    L.mlens_trim_memory.restype = ci
     L.mlens_destroy.argtypes = [vp]
     L.mlens_destroy.restype = None
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
@@ -94,6 +96,11 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
         getattr(L, name).restype = ci
     _libs[key] = L
     return L
+
+
+def trim_memory(ablations: bool = False):
+    """mlens_trim_memory: release the device blocks that destroyed handles left in the library's pool (current device)."""
+    _check(lib(ablations).mlens_trim_memory(), lib(ablations))
 
 
 def _check(rc: int, L=None):

@@ -573,3 +573,23 @@ def test_two_streams_on_one_handle(ml, oracle):
             st = h.stats()
             assert st["rays_total"] == g.n1 * g.n2 and st["rays_in_map"] == st_full["rays_in_map"]
             assert torch.equal(cnt, full)
+
+
+def test_handles_recycle_pooled_memory_and_trim(ml):
+    # device blocks of destroyed handles stay in the library's pool and are reused; mlens_trim_memory returns them
+    cfg = dataclasses.replace(fields.CONFIGS[1], npix=512, sub=2)
+    xy, m = fields.lens_field(cfg)
+    torch.cuda.synchronize()
+    maps = []
+    for _ in range(4):
+        with ml.Mlens.from_config(cfg, xy, m) as h:
+            c, mg, st = h.shoot_host()
+            maps.append(c.copy())
+    assert all(np.array_equal(maps[0], c) for c in maps[1:])
+    free0, _ = torch.cuda.mem_get_info()
+    ml.trim_memory()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 >= free0  # the cached result buffers (2 x 1 MB here) went back; nothing is in use any more
+    with ml.Mlens.from_config(cfg, xy, m) as h:  # and the pool still works after a trim
+        c, _, _ = h.shoot_host()
+    assert np.array_equal(c, maps[0])
