@@ -62,16 +62,16 @@ def case_near_overflow():
     with mlens.Mlens.from_config(cfg, cluster, m) as h:
         g = h.geometry
         cnt = torch.zeros((npix, npix), dtype=torch.int32, device="cuda")
-        h.shoot_block(g.n1 // 2 - 64, g.n2 // 2 - 64, 128, 128, count=cnt)
+        h.shoot_block(0, 0, g.n1, g.n2, count=cnt)
         st = h.stats()
-    assert st["rays_total"] == 128 * 128
-    return f"near-list overflow: 128x128 rays, 60 lenses inside one tile, in_map {st['rays_in_map']}"
+    assert st["rays_total"] == g.n1 * g.n2
+    return f"near-list overflow: {g.n1}x{g.n2} rays, 60 lenses inside one tile, in_map {st['rays_in_map']}"
 
 
 def case_mpd_and_index():
     npix = 256
     u = fields.uniform01(7, 0, npix * npix)
-    count = (u * u * 60000).astype(np.int32)  # > 48 Ki distinct bins in play: shared-memory bins + global 64-bit bins
+    count = (u * u * 60000).astype(np.int32).reshape(npix, npix)  # > 48 Ki distinct bins in play: shared-memory bins + global 64-bit bins
     with mlens.Mlens(0.3, 0.2, 0.0, 4.0, npix, 4.0 / npix / 2, np.zeros((1, 2), np.float32)) as h:
         c = torch.from_numpy(count).cuda()
         n_bins = int(count.max()) + 2
