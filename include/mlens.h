@@ -104,7 +104,10 @@ int mlens_shoot(mlens_t* h, int* count_dev, float* mag_dev, void* cuda_stream, m
  *   count_dev   DEVICE npix*npix int32, or NULL (no binning)
  *   ray_y_dev   DEVICE ni*nj*2 doubles or NULL: source position of ray (ii, jj) at [2*(jj*ni+ii)], [.. + 1]
  *   ray_pix_dev DEVICE ni*nj int32 or NULL: pixel id, -1 = outside the map, -2 = non-finite
- * Asynchronous on `cuda_stream`.  MLENS_EINVAL if the block is not inside [0,n1) x [0,n2). */
+ * Asynchronous on `cuda_stream`.  MLENS_EINVAL if the block is not inside [0,n1) x [0,n2); MLENS_ERANGE (also from
+ * mlens_shoot) if ray_spacing is so small against the lens distances or masses that the FP32 loop, which works in units
+ * of ray_spacing, would leave the FP32 range ((|lens coordinate| + rectangle)/ray_spacing > ~2e18, or m/ray_spacing^2 >
+ * 1e37) — far outside any physical configuration. */
 int mlens_shoot_block(mlens_t* h, long long i0, long long j0, long long ni, long long nj, int* count_dev,
                       double* ray_y_dev, int* ray_pix_dev, void* cuda_stream);
 

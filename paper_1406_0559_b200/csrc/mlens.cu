@@ -175,6 +175,7 @@ struct mlens {
     // options
     int opt_kernel, opt_binning, opt_ctas_per_sm, opt_shared, opt_rays, opt_tile_x, opt_shared_pairs;
     double lens_extent;                // max |coordinate| over the lens list (guards the shared-reciprocal products)
+    double mass_max;                   // largest lens mass (guards the FP32 range of the lattice-unit loop)
 };
 
 namespace {
@@ -310,6 +311,9 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         int shared = h->opt_shared_pairs;
         const double zmax = (h->lens_extent + std::fmax(h->geo.a1, h->geo.a2)) / h->d;  // per axis, lattice units
         if (shared > 0 && 4.0 * zmax * zmax * zmax * zmax > 1.0e37) shared = 0;
+        // the loop itself forms |w|^2 <= 2 zmax^2 and c conj(w) ~ m / d^2 in FP32
+        if (P.n_lens > 0 && (2.0 * zmax * zmax > 1.0e37 || h->mass_max / (h->d * h->d) > 1.0e37))
+            return fail(MLENS_ERANGE, "ray_spacing %g is too small for the FP32 lattice-unit loop (lens distances / spacing up to %g)", h->d, zmax);
         const int code = h->opt_rays * 10000 + h->opt_tile_x * 10 + shared;
         // the default launch (run-combining REDs into a count map, no per-ray outputs) has its own, leaner instantiation
         const bool runs = h->opt_binning == mlk::BIN_RUNS && count != nullptr && ray_y == nullptr && ray_pix == nullptr;
@@ -438,8 +442,10 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     h->device = dev; h->sm_count = sm_count;
     h->opt_kernel = 1; h->opt_binning = mlk::BIN_RUNS; h->opt_ctas_per_sm = 0; h->opt_shared = 0; h->opt_rays = kProdRays;
     h->opt_tile_x = kProdTileX; h->opt_shared_pairs = kProdSharedPairs;
-    for (long long k = 0; k < n_lens; ++k)
+    for (long long k = 0; k < n_lens; ++k) {
         h->lens_extent = std::fmax(h->lens_extent, std::fmax(std::fabs((double)packed[(size_t)k].x), std::fabs((double)packed[(size_t)k].y)));
+        h->mass_max = std::fmax(h->mass_max, (double)packed[(size_t)k].z);
+    }
 
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = dev_alloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));

@@ -575,6 +575,16 @@ def test_two_streams_on_one_handle(ml, oracle):
             assert torch.equal(cnt, full)
 
 
+def test_spacing_below_the_fp32_range_is_refused(ml):
+    # lattice units divide every length by d: lens distances / d beyond ~2e18 would overflow |w|^2 in FP32 -> MLENS_ERANGE
+    # from the launch (never a silently wrong map)
+    xy = np.array([[3.0e5, 0.0]], np.float32)
+    with ml.Mlens(0.3, 0.1, 0.0, 1.0e-12, 4, 1.0e-14, xy) as h:
+        with pytest.raises(ml.MlensError) as e:
+            h.shoot()
+        assert e.value.code == ml.ERANGE
+
+
 def test_handles_recycle_pooled_memory_and_trim(ml):
     # device blocks of destroyed handles stay in the library's pool and are reused; mlens_trim_memory returns them
     cfg = dataclasses.replace(fields.CONFIGS[1], npix=512, sub=2)
