@@ -230,7 +230,8 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream);
  *                  the parity tolerances: the evidence for the difference form; <= 12000 lenses), 3 = tensor-pipe
  *                  experiment (r^2, Re, Im of every interaction from tcgen05 TF32 MMAs; slower than kernel 1 and NOT
  *                  deterministic: its per-ray partial sums meet in shared-memory float atomics), 4 = the round-1
- *                  production kernel (A/B baseline; its loop variant "shared_rcp" 0..2)
+ *                  production kernel (A/B baseline; its loop variant "shared_rcp" 0..2), 5 = kernel 3 slimmed to 8 consumer
+ *                  warps (288 threads) so that it can share an SM with a CUDA-core CTA (bench.py --corun)
  *   "rays_per_thread" 8 | 16, "tile_x" 64 | 48 | 32 (8 rays only), "shared_pairs" 0..4: the sweep grid of kernel 1
  * Returns MLENS_EINVAL for an unknown key or value. */
 int mlens_set_option(mlens_t* h, const char* key, long long value);

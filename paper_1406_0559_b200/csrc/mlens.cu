@@ -237,7 +237,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         return MLENS_OK;
     }
 
-    if (h->opt_kernel == 3) {  // experimental: pre-reciprocal terms from the tensor pipe (shoot_umma_kernel.cuh)
+    if (h->opt_kernel == 3 || h->opt_kernel == 5) {  // experimental: pre-reciprocal terms from the tensor pipe (shoot_umma_kernel.cuh)
         if (!h->umma_A_dev) {
             std::vector<float> A((size_t)mlk::kUmBlocks * mlk::kUmRays * 8, 0.f);
             auto tf32 = [](float x) { uint32_t b; memcpy(&b, &x, 4); b = (b + 0x1000u) & 0xffffe000u; memcpy(&x, &b, 4); return x; };
@@ -254,13 +254,19 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
             MLENS_CUDA(cudaMemcpy(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice));
         }
         P.umma_A = h->umma_A_dev;
-        const size_t smem = (size_t)mlk::kUmBlocks * mlk::kUmABlockBytes + (size_t)(mlk::kUmSuper / mlk::kUmLenses) * mlk::kUmChunkBytes +
+        // kernel 3: 16 consumer warps, 512-lens super-chunks; kernel 5: the slim variant (8 consumer warps, 256-lens
+        // super-chunks: 288 threads x 96 registers, 186 KB) that can share an SM with one CTA of the production kernel
+        const bool slim = h->opt_kernel == 5;
+        const int super = slim ? 256 : 512, cons = slim ? 8 : 16;
+        const size_t smem = (size_t)mlk::kUmBlocks * mlk::kUmABlockBytes + (size_t)(super / mlk::kUmLenses) * mlk::kUmChunkBytes +
                             (size_t)mlk::kTile * mlk::kTile * sizeof(float2) + sizeof(mlk::UmmaShared) + 1024;
         const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
         long long grid = h->sm_count;
         if (grid > n_tiles) grid = n_tiles;
-        MLENS_CUDA(cudaFuncSetAttribute(mlk::shoot_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        mlk::shoot_umma_kernel<<<(unsigned)grid, mlk::kUmThreads, smem, st>>>(P);
+        void (*uk)(const mlk::ShootParams) = slim ? mlk::shoot_umma_kernel<8, 256> : mlk::shoot_umma_kernel<16, 512>;
+        MLENS_CUDA(cudaFuncSetAttribute(uk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        MLENS_CUDA(cudaFuncSetAttribute(uk, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+        uk<<<(unsigned)grid, 32 * (cons + 1), smem, st>>>(P);
         MLENS_CUDA(cudaGetLastError());
         return MLENS_OK;
     }
@@ -342,6 +348,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     long long grid = (long long)h->sm_count * ctas;
     if (grid > n_tiles) grid = n_tiles;
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     kern<<<(unsigned)grid, threads, smem, st>>>(P);
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
@@ -531,7 +538,7 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
         return fail(MLENS_EINVAL, "option %s=%lld needs the MLENS_ABLATIONS build of the library", key, value);
 #endif
     if (!strcmp(key, "kernel")) {
-        if (value < 0 || value > 4) return fail(MLENS_EINVAL, "kernel must be 0..4");
+        if (value < 0 || value > 5) return fail(MLENS_EINVAL, "kernel must be 0..5");
         h->opt_kernel = (int)value;
     } else if (!strcmp(key, "tile_x")) {
         if (value != 64 && value != 48 && value != 32) return fail(MLENS_EINVAL, "tile_x must be 64, 48 or 32");

@@ -25,10 +25,11 @@ namespace mlk {
 constexpr int kUmRays = 128;        // rays per MMA (M)
 constexpr int kUmLenses = 64;       // lenses per MMA (N = 3 * 64)
 constexpr int kUmN = 3 * kUmLenses;
-constexpr int kUmSuper = 512;       // lenses per super-chunk resident in shared memory
+constexpr int kUmSuperMax = 512;    // lenses per super-chunk resident in shared memory (template parameter kSuper: 512 or 256)
 constexpr int kUmBlocks = kTile * kTile / kUmRays;  // 32 ray blocks per tile
-constexpr int kUmConsumers = 16;    // consumer warps: 4 TMEM lane quadrants x 4 lens quarters of every MMA
-constexpr int kUmThreads = 32 * (kUmConsumers + 1);
+constexpr int kUmConsumersMax = 16;  // consumer warps (template parameter kCons): 16 = 2 groups x 4 TMEM lane quadrants x 2 halves of
+                                    // a chunk's lenses; 8 = 2 groups x 4 quadrants, every warp takes the whole chunk (the slim variant
+                                    // that can share an SM with a CTA of the production kernel: 288 threads, 96 registers)
 constexpr int kUmChunkBytes = kUmN * 8 * 4;         // 6144: one B chunk (192 rows x K = 8)
 constexpr int kUmABlockBytes = kUmRays * 8 * 4;     // 4096: one A block
 
@@ -69,13 +70,18 @@ struct __align__(16) UmmaShared {
     uint32_t tmem_base;
     int near_n;
     long long next_tile;
-    double part[kUmThreads / 32][2];
+    double part[kUmConsumersMax + 1][2];
     double near_zx[kNearMax], near_zy[kNearMax], near_m[kNearMax];
     unsigned long long ctr[3];
 };
 
 
-__global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootParams P) {
+template <int kCons, int kSuper>
+__global__ void __maxnreg__(kCons == 8 ? 112 : 96) shoot_umma_kernel(const ShootParams P) {
+    constexpr int kUmConsumers = kCons, kUmThreads = 32 * (kCons + 1), kUmSuper = kSuper;
+    constexpr int kParts = kCons / 8;        // warps that share one TMEM lane quadrant of a group
+    constexpr int kHf = 4 / kParts;          // 16-lens sub-blocks of a chunk per warp
+    constexpr int kBarThreads = 32 * kCons;  // both consumer groups take part in each named barrier
     extern __shared__ __align__(1024) unsigned char um_smem[];
     unsigned char* sA = um_smem;                                                     // 32 ray blocks x 4 KB
     unsigned char* sB = sA + kUmBlocks * kUmABlockBytes;                             // 8 lens chunks x 6 KB
@@ -107,7 +113,7 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
     // Ping-pong of the arithmetic phase between the two consumer groups (named barriers 1 and 2, 512 threads each):
     // a group may only do its MUFU/FMA work while the other one waits for / reads its next accumulator, so the two can
     // never fall into lock-step (both computing, then both waiting, with the MUFU idle a third of the time).
-    if (!is_control && (warp >> 3) == 1) asm volatile("bar.arrive 1, 512;" ::: "memory");
+    if (!is_control && warp / (4 * kParts) == 1) asm volatile("bar.arrive 1, %0;" ::"n"(kBarThreads) : "memory");
     const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
     const int n_super = P.n_lens > 0 ? (P.n_lens + kUmSuper - 1) / kUmSuper : 0;
     uint32_t seq = 0;  // MMA sequence number: buffer seq & 1, use (seq >> 1) of that buffer; same count in every warp
@@ -195,7 +201,7 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
                 // Two consumer groups of 8 warps work on alternate chunks (TMEM buffer = group): while one group is in its
                 // TMEM-read phase (64 B/clk per sub-partition: the binding resource of this kernel) the other is in its
                 // MUFU/FMA phase.  Within a group: 4 lane quadrants x 2 halves of the chunk's 64 lenses.
-                const int group = warp >> 3, quad = warp & 3, part = (warp >> 2) & 1;
+                const int group = warp / (4 * kParts), quad = warp & 3, part = (warp >> 2) % kParts;
                 for (int rb = 0; rb < kUmBlocks; ++rb) {
                     float2 S[4];  // (S_re, S_im) partial sums, four independent chains
 #pragma unroll
@@ -206,19 +212,19 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
                         mbar_wait_parity(&sh.full[buf], use & 1u);
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t tbase = tmem_base + ((uint32_t)(quad * 32) << 16) + buf * kUmN;
-#pragma unroll
-                        for (int hf = 0; hf < 2; ++hf) {
-                            const int l16 = part * 2 + hf;  // which 16 of the chunk's 64 lenses
+#pragma unroll(kHf == 2 ? 2 : 1)
+                        for (int hf = 0; hf < kHf; ++hf) {
+                            const int l16 = part * kHf + hf;  // which 16 of the chunk's 64 lenses
                             float r2[16], pq[32];
                             tmem_ld16(tbase + l16 * 16, r2);
                             tmem_ld16(tbase + kUmLenses + l16 * 32, pq);
                             tmem_ld16(tbase + kUmLenses + l16 * 32 + 16, pq + 16);
                             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
                             if (hf == 0) {
-                                if (group == 0) asm volatile("bar.sync 1, 512;" ::: "memory");
-                                else asm volatile("bar.sync 2, 512;" ::: "memory");
+                                if (group == 0) asm volatile("bar.sync 1, %0;" ::"n"(kBarThreads) : "memory");
+                                else asm volatile("bar.sync 2, %0;" ::"n"(kBarThreads) : "memory");
                             }
-                            if (hf == 1) {
+                            if (hf == kHf - 1) {
                                 // everything of this buffer is in registers: hand it back before the arithmetic
                                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                                 __syncwarp();
@@ -237,8 +243,8 @@ __global__ void __launch_bounds__(kUmThreads, 1) shoot_umma_kernel(const ShootPa
                                 S[3] = __ffma2_rn(make_float2(pq[2 * j + 6], pq[2 * j + 7]), make_float2(RCb.y, RCb.y), S[3]);
                             }
                         }
-                        if (group == 0) asm volatile("bar.arrive 2, 512;" ::: "memory");
-                        else asm volatile("bar.arrive 1, 512;" ::: "memory");
+                        if (group == 0) asm volatile("bar.arrive 2, %0;" ::"n"(kBarThreads) : "memory");
+                        else asm volatile("bar.arrive 1, %0;" ::"n"(kBarThreads) : "memory");
                     }
                     const int ray = rb * kUmRays + quad * 32 + lane;
                     atomicAdd(&sS[ray].x, (S[0].x + S[1].x) + (S[2].x + S[3].x));
