@@ -575,6 +575,23 @@ def test_two_streams_on_one_handle(ml, oracle):
             assert torch.equal(cnt, full)
 
 
+def test_shipped_library_one_reciprocal_per_ray_option(ml, oracle):
+    # the shipped library's two instantiations (two shared ray pairs — the default — and one MUFU.RCP per ray, which is also
+    # the automatic fallback for extreme coordinates) through the public option, both against the oracle
+    cfg = dataclasses.replace(fields.CONFIGS[4], npix=200, sub=3)
+    xy, m = fields.lens_field(cfg)
+    ref = oracle.shoot_block(*_args(cfg), xy, m)
+    maps = {}
+    with ml.Mlens.from_config(cfg, xy, m) as h:
+        for sp in (2, 0):
+            h.set_option("shared_pairs", sp)
+            c, _, st = h.shoot(want_mag=False)
+            maps[sp] = c.cpu().numpy().astype(np.int64)
+            l1 = int(np.abs(maps[sp] - ref["count"]).sum())
+            assert st["rays_total"] == ref["stats"]["rays_total"] and l1 <= max(2, TOL_L1 * ref["stats"]["rays_in_map"]), (sp, l1)
+    assert np.abs(maps[0] - maps[2]).sum() <= max(4, 2 * TOL_L1 * ref["stats"]["rays_in_map"])
+
+
 def test_spacing_below_the_fp32_range_is_refused(ml):
     # lattice units divide every length by d: lens distances / d beyond ~2e18 would overflow |w|^2 in FP32 -> MLENS_ERANGE
     # from the launch (never a silently wrong map)
