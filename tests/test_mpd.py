@@ -56,7 +56,8 @@ def test_p11_mpd_brute_force_invariants_and_clamping(oracle):
 # GPU parity
 # ---------------------------------------------------------------------------------------------------------------
 @pytest.mark.gpu
-@pytest.mark.parametrize("npix,n_bins,hi", [(64, 4096, 3000), (250, 100, 5000), (1023, 20000, 19000), (1, 2, 5), (2048, 9000, 40000), (512, 70000, 69000)])
+@pytest.mark.parametrize("npix,n_bins,hi", [(64, 4096, 3000), (250, 100, 5000), (1023, 20000, 19000), (1, 2, 5), (2048, 9000, 40000), (512, 70000, 69000),
+                                            (4096, 30000, 29000), (130, 38000, 37000)])
 def test_mlens_mpd_matches_the_oracle_bit_for_bit(oracle, npix, n_bins, hi):
     import torch
 
@@ -79,6 +80,10 @@ def test_mlens_mpd_matches_the_oracle_bit_for_bit(oracle, npix, n_bins, hi):
         for k in ("n_pixels", "sum_count", "n_clamped", "min_count", "max_count"):
             assert st[k] == ref[k], k
         assert st["mean_count"] == ref["mean_count"] and st["mean_mu"] == ref["mean_mu"]
+        # an all-equal map: the flat-region vote (one add of 128 per warp) instead of 32-way same-address atomics
+        flat = torch.full((npix, npix), 7, dtype=torch.int32, device="cuda")
+        hf, sf = h.mpd(flat, n_bins)
+        assert int(hf[min(7, n_bins - 1)].item()) == npix * npix and sf["sum_count"] == 7 * npix * npix
 
 
 @pytest.mark.gpu
