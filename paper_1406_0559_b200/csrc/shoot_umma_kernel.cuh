@@ -33,7 +33,7 @@ constexpr int kUmConsumersMax = 16;  // consumer warps (template parameter kCons
 constexpr int kUmChunkBytes = kUmN * 8 * 4;         // 6144: one B chunk (192 rows x K = 8)
 constexpr int kUmABlockBytes = kUmRays * 8 * 4;     // 4096: one A block
 
-// canonical K-major no-swizzle UMMA layout for 4-byte elements (see umma_probe.cu)
+// canonical K-major no-swizzle UMMA layout for 4-byte elements (probed in round 1: profiles/r1e_umma_probe.md)
 __host__ __device__ inline int umma_off_bytes(int r, int k) { return (r % 8) * 16 + (r / 8) * 256 + (k / 4) * 128 + (k % 4) * 4; }
 
 __device__ __forceinline__ uint64_t umma_smem_desc(uint32_t saddr) {
