@@ -132,6 +132,44 @@ int mlens_magnification(mlens_t* h, const int* count_dev, float* mag_dev, void* 
 int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, int n_bins, void* cuda_stream,
               mlens_map_stats* stats);
 
+/* The MPD for callers that cannot allocate memory.
+ *
+ * mlens_mpd works on a handle, and both mlens_create and the first mlens_mpd on a handle allocate (device blocks for the
+ * lens list, the counters and the per-CTA histogram slices; pinned host blocks for the statistics).  Some users of this
+ * library cannot do that at the point where they want a map's statistics: a survey worker or a server that gave all of
+ * its device memory to one allocator when it started (so that a later cudaMalloc fails, or breaks a memory budget its
+ * scheduler enforces), or a loop that analyses finished maps while the next map is being shot on another stream (an
+ * allocation synchronises the whole device and would stall the shooting kernel).  This entry point computes the same
+ * histogram and the same statistics with the same kernels, takes no handle, and calls no cudaMalloc, cudaMallocHost,
+ * cudaFree or other allocating routine: its scratch is a fixed array that is part of the library image.
+ *
+ *   count_dev  DEVICE n_pixels int32, 16-byte aligned (a finished count map; any shape — only the pixel count matters)
+ *   n_pixels   >= 1
+ *   n_avg      N_avg of the map, (pixel/ray_spacing)^2; only used for stats->mean_mu (must be > 0 if stats != NULL)
+ *   hist_dev   DEVICE n_bins unsigned 64-bit, caller-owned; ZEROED by the call, then filled exactly as by mlens_mpd
+ *              (counts >= n_bins-1 are clamped into the last bin)
+ *   n_bins     2 .. MLENS_MPD_STATIC_MAX_BINS.  More bins: MLENS_ERANGE — use mlens_mpd, or clamp
+ *   stats      HOST or NULL, as in mlens_mpd: NULL = asynchronous on `cuda_stream`; otherwise the stream is
+ *              synchronised and *stats filled (copied into the caller's struct directly, no pinned mirror)
+ *
+ * The scratch: 148 x MLENS_MPD_STATIC_MAX_BINS 32-bit bins + 64 bytes = 4.6 MiB of device memory, held by EVERY GPU on
+ * which the process uses this library, from the moment the library is loaded there until the process exits — whether or
+ * not this function is ever called.  That is the price of never allocating, and the reason for the limit on n_bins.
+ * ONE array per GPU is shared by all callers in the process, and it keeps what the last call left in it.  The call
+ * clears the part that must start at zero itself (on `cuda_stream`), so calls that are ordered one after the other —
+ * same stream, or streams ordered by events — are independent of each other.  Two calls that may run on the GPU at the
+ * same time (different streams without ordering, different host threads) RACE on the array and return wrong
+ * histograms; nothing detects this.  Order them, or use handles and mlens_mpd for concurrent work.
+ *
+ * The first call on each device looks up the array's device address (once per device, with that device current) and
+ * checks that the device is an sm_100 part; make that first call during set-up, before any stream capture is begun.
+ * Later calls only enqueue two memsets and two kernels.
+ * Errors: MLENS_EINVAL (NULL pointers, n_pixels < 1, n_bins < 2, bad n_avg with stats), MLENS_ERANGE (n_bins beyond the
+ * limit), MLENS_ECUDA (no sm_100 device, CUDA failure). */
+#define MLENS_MPD_STATIC_MAX_BINS 8192
+int mlens_mpd_static(const int* count_dev, long long n_pixels, double n_avg, unsigned long long* hist_dev, int n_bins,
+                     void* cuda_stream, mlens_map_stats* stats);
+
 /* Indexed maps: "The index file will hold all the distinct ray-count values,
  * each matched to an index running from zero to the maximum number of distinct ray-counts in the map.  The indexed map
  * will have its pixel ray-count values replaced by the appropriate index" — stored in 16 bits, halving the map.

@@ -877,3 +877,103 @@ int mlens_shoot_host(mlens_t* h, int* count_host, float* mag_host, mlens_stats* 
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// mlens_mpd_static: the MPD of a count map for callers that must not allocate (include/mlens.h has the full contract).
+//
+// mlens_mpd needs a handle (mlens_create allocates the lens list, counters, events) and on first use takes its per-CTA
+// histogram slices and a pinned statistics mirror from cudaMalloc / cudaMallocHost.  A process whose device memory is
+// already spoken for — everything handed to one caching allocator at start-up, a fixed budget set by a job scheduler —
+// or that computes map statistics next to running shooting kernels, where an allocation's device-wide synchronisation
+// would stall them, cannot afford that.  Here the same two kernels (mpd_kernel, mpd_reduce_kernel) run with their
+// scratch in the file-scope array below, which exists on every GPU that loads the library from load to exit.
+//
+// Size: kStaticMaxCtas slices of kStaticMaxBins 32-bit bins (148 x 8192 x 4 B = 4.6 MiB) + one MapStatsDev.
+// ---------------------------------------------------------------------------------------------------------------
+namespace {
+constexpr int kStaticMaxBins = MLENS_MPD_STATIC_MAX_BINS;  // multiple of 1024 (the kernels' fill / flush loops)
+constexpr int kStaticMaxCtas = 148;                        // one persistent CTA per SM of a B200
+constexpr size_t kStaticSliceWords = (size_t)kStaticMaxCtas * kStaticMaxBins;
+static_assert(kStaticMaxBins % 1024 == 0 && kStaticMaxBins <= mlk::kMpdSmemBinsMax, "static MPD bins");
+static_assert(sizeof(mlk::MapStatsDev) <= 64 && (kStaticSliceWords * 4) % 256 == 0, "static MPD scratch layout");
+}  // namespace
+
+// [0, kStaticSliceWords): per-CTA histogram slices; then 16 words for the MapStatsDev accumulator.
+// In HOST code this name is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress below.
+static __device__ __align__(256) unsigned int g_mpd_static_scratch[kStaticSliceWords + 16];
+
+namespace {
+std::mutex g_static_mutex;
+unsigned int* g_static_ptr[64];  // device address of g_mpd_static_scratch on each device, looked up once per device
+int g_static_sm_count[64];
+
+// Once per device, with that device current: look up the array's device address.  No allocation; the first call on a
+// device may make the runtime load the library's module, which is why it should happen outside any stream capture.
+int static_scratch(unsigned int** ptr, int* sm_count) {
+    int dev = -1;
+    MLENS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(MLENS_ECUDA, "device ordinal %d is outside 0..63", dev);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        int cc_major = 0, cc_minor = 0, sms = 0;
+        MLENS_CUDA(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+        MLENS_CUDA(cudaDeviceGetAttribute(&cc_minor, cudaDevAttrComputeCapabilityMinor, dev));
+        MLENS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (cc_major != 10) return fail(MLENS_ECUDA, "device %d is sm_%d%d; this library is built for sm_100a only", dev, cc_major, cc_minor);
+        void* p = nullptr;
+        MLENS_CUDA(cudaGetSymbolAddress(&p, g_mpd_static_scratch));
+        if (!p) return fail(MLENS_ECUDA, "cudaGetSymbolAddress returned a NULL address for the static MPD scratch");
+        g_static_sm_count[dev] = sms;
+        g_static_ptr[dev] = static_cast<unsigned int*>(p);
+    }
+    *ptr = g_static_ptr[dev];
+    *sm_count = g_static_sm_count[dev];
+    return MLENS_OK;
+}
+}  // namespace
+
+extern "C" int mlens_mpd_static(const int* count_dev, long long n_pixels, double n_avg, unsigned long long* hist_dev,
+                                int n_bins, void* cuda_stream, mlens_map_stats* stats) {
+    if (!count_dev || !hist_dev) return fail(MLENS_EINVAL, "NULL argument");
+    if (n_pixels < 1) return fail(MLENS_EINVAL, "n_pixels must be >= 1");
+    if (n_bins < 2) return fail(MLENS_EINVAL, "n_bins must be >= 2");
+    if (n_bins > kStaticMaxBins)
+        return fail(MLENS_ERANGE, "n_bins = %d is beyond the %d bins that the static scratch of mlens_mpd_static holds; "
+                    "use mlens_mpd (which allocates) for finer histograms", n_bins, kStaticMaxBins);
+    if (stats && (!std::isfinite(n_avg) || !(n_avg > 0))) return fail(MLENS_EINVAL, "n_avg must be finite and > 0 when stats are requested");
+    unsigned int* scratch = nullptr;
+    int sm_count = 0;
+    if (int rc = static_scratch(&scratch, &sm_count)) return rc;
+    unsigned int* partial = scratch;
+    mlk::MapStatsDev* st_dev = reinterpret_cast<mlk::MapStatsDev*>(scratch + kStaticSliceWords);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // What must start at zero: the statistics accumulator (atomic sums / maxima) and the caller's bins.  The slices need
+    // no clearing although they keep the previous call's contents: every CTA overwrites its whole slice [0, smem_bins)
+    // and the reduction reads exactly the slices of the CTAs of THIS launch.
+    MLENS_CUDA(cudaMemsetAsync(st_dev, 0, sizeof(mlk::MapStatsDev), st));
+    MLENS_CUDA(cudaMemsetAsync(hist_dev, 0, sizeof(unsigned long long) * (size_t)n_bins, st));
+    const int smem_bins = (n_bins + 1023) & ~1023;  // <= kStaticMaxBins: all bins live in shared memory
+    long long blocks = (n_pixels / 4 + mlk::kMpdThreads - 1) / mlk::kMpdThreads;
+    if (blocks > sm_count) blocks = sm_count;
+    if (blocks > kStaticMaxCtas) blocks = kStaticMaxCtas;
+    if (blocks < 1) blocks = 1;
+    const size_t smem = sizeof(unsigned int) * (size_t)smem_bins;
+    MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n_pixels, hist_dev, n_bins, smem_bins, partial, st_dev);
+    MLENS_CUDA(cudaGetLastError());
+    mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(partial, (int)blocks, smem_bins, hist_dev, n_bins, st_dev);
+    MLENS_CUDA(cudaGetLastError());
+    if (stats) {
+        mlk::MapStatsDev host;  // pageable stack memory: the copy is staged by the driver, nothing is allocated here
+        MLENS_CUDA(cudaMemcpyAsync(&host, st_dev, sizeof(host), cudaMemcpyDeviceToHost, st));
+        MLENS_CUDA(cudaStreamSynchronize(st));
+        stats->n_pixels = n_pixels;
+        stats->sum_count = (long long)host.sum_count;
+        stats->n_clamped = (long long)host.n_clamped;
+        stats->min_count = 0x7fffffff - host.inv_min_count;
+        stats->max_count = host.max_count;
+        stats->mean_count = (double)stats->sum_count / (double)n_pixels;
+        stats->mean_mu = stats->mean_count / n_avg;
+    }
+    return MLENS_OK;
+}

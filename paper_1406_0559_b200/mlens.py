@@ -68,6 +68,7 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_shoot_host.argtypes = [vp, vp, vp, ctypes.POINTER(Stats)]
     L.mlens_magnification.argtypes = [vp, vp, vp, vp]
     L.mlens_mpd.argtypes = [vp, vp, vp, ci, vp, ctypes.POINTER(MapStats)]
+    L.mlens_mpd_static.argtypes = [vp, ll, dbl, vp, ci, vp, ctypes.POINTER(MapStats)]
     L.mlens_index_map.argtypes = [vp, vp, vp, ci, vp, vp, ctypes.POINTER(ci)]
     L.mlens_unindex_map.argtypes = [vp, vp, vp, ci, vp, vp]
     L.mlens_bits_needed.argtypes = [ctypes.c_ulonglong]
@@ -92,7 +93,7 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
                  "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option", "mlens_bits_needed",
-                 "mlens_pack_map", "mlens_unpack_map", "mlens_mpd_rebin", "mlens_convolve_prepare"):
+                 "mlens_pack_map", "mlens_unpack_map", "mlens_mpd_rebin", "mlens_convolve_prepare", "mlens_mpd_static"):
         getattr(L, name).restype = ci
     _libs[key] = L
     return L
@@ -113,6 +114,30 @@ def _stream_ptr(stream=None):
 
     s = stream if stream is not None else torch.cuda.current_stream()
     return ctypes.c_void_p(s.cuda_stream)
+
+
+MPD_STATIC_MAX_BINS = 8192  # MLENS_MPD_STATIC_MAX_BINS of include/mlens.h
+
+
+def mpd_static(count, n_bins, n_avg, hist, stream=None, sync=True, ablations=False):
+    """mlens_mpd_static: the MPD histogram and map statistics of ``count`` without a handle and without any allocation
+    inside the library — for programs that have no device memory left to give (everything reserved by one allocator, a
+    fixed budget) or that must not pay an allocation's device-wide synchronisation while other streams are busy.
+
+    ``hist`` is the caller's int64 [n_bins] device tensor (n_bins <= MPD_STATIC_MAX_BINS); this wrapper allocates nothing
+    either.  All calls in the process share one scratch array per GPU: calls that could overlap on the GPU race, so keep
+    them on one stream or order the streams.  Make the first call on a device before starting any stream capture.
+    Returns (hist, stats dict or None when sync=False)."""
+    import torch
+
+    assert count.is_cuda and count.dtype == torch.int32 and count.is_contiguous()
+    assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous() and hist.numel() == int(n_bins)
+    L = lib(ablations)
+    ms = MapStats() if sync else None
+    _check(L.mlens_mpd_static(ctypes.c_void_p(count.data_ptr()), int(count.numel()), float(n_avg),
+                              ctypes.c_void_p(hist.data_ptr()), int(n_bins), _stream_ptr(stream),
+                              ctypes.byref(ms) if sync else None), L)
+    return hist, (ms.as_dict() if sync else None)
 
 
 class Mlens:
