@@ -115,9 +115,13 @@ def oracle_block_for(cfg, n1, n2, n_lens, target_s, rate_guess):
     return ((n1 - side) // 2, (n2 - side) // 2, side, side)
 
 
+_ORACLE_THREADS = 0  # 0 = OpenMP's own choice; the reference arm under a multi-rank launcher sets it (see run_reference)
+
+
 def oracle_time_block(oracle, cfg, xy, m, block):
     t0 = time.perf_counter()
-    r = oracle.shoot_block(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, xy, m, block=block)
+    r = oracle.shoot_block(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing, xy, m, block=block,
+                           n_threads=_ORACLE_THREADS)
     dt = time.perf_counter() - t0
     return dt, r["stats"]["rays_total"]
 
@@ -148,10 +152,17 @@ def run_cpu_baseline(cfg, xy, m, target_s=15.0):
 def run_reference(args):
     """--impl reference: the oracle on the host cores, K timed steps of a bounded sample each (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
+        print(f"bench.py: rank {os.environ['RANK']} of {os.environ.get('WORLD_SIZE', '?')}: idle (the reference arm runs on rank 0 only)",
+              file=sys.stderr, flush=True)
         return
     import oracle
 
     oracle.lib()
+    global _ORACLE_THREADS
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        # torch.distributed.run exports OMP_NUM_THREADS=1 to every rank; here the other ranks idle, so rank 0 takes the
+        # host cores this process may run on — the same machine share the N = 1 reference run gets
+        _ORACLE_THREADS = len(os.sched_getaffinity(0))
     cfg = fields.CONFIGS[args.config]
     xy, m = fields.lens_field(cfg)
     g = oracle.geometry(cfg.kappa, cfg.gamma, cfg.s, cfg.map_side, cfg.npix, cfg.ray_spacing)
@@ -175,7 +186,8 @@ def run_reference(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(args.config, cfg, len(m), g.n1, g.n2), "sample": sample},
             "rays_per_s": rays / dt,
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": _ORACLE_THREADS or oracle.max_threads(), "kind": "oracle",
+                             "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -334,7 +346,8 @@ def run_ours(args):
     in_map = st["rays_in_map"]
 
     # end to end through the C ABI with host buffers: create (H2D lens list) + shoot + D2H maps + destroy
-    e2e_steps = max(1, min(args.steps, 2))
+    # maps of seconds: two end-to-end maps; maps shorter than a second: as many as --steps (capped), a usable statistic
+    e2e_steps = max(1, min(args.steps, 2 if ms_total / max(1, args.steps) >= 1000.0 else 50))
     h.close()
     barrier()
     e2e_kernel_ms = []
@@ -610,6 +623,64 @@ def run_convolve(args):
           flush=True)
 
 
+# -----------------------------------------------------------------------------------------------------------------
+# N > 1: one process per GPU.  The driver starts the ranks itself (torch.distributed.run); called plainly as
+# `python bench.py --gpus N`, bench.py re-executes itself under the same launcher so that N ranks really run.
+# -----------------------------------------------------------------------------------------------------------------
+def _free_port() -> int:
+    import socket
+
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        return sock.getsockname()[1]
+
+
+def launch_ranks(args) -> int:
+    """`--gpus N` (N > 1) without a launcher's environment: start N ranks of this very command line under
+    `python -m torch.distributed.run` on 127.0.0.1 and a free port.  Never falls back to one rank: the GPU arms fail
+    loudly when fewer than N devices are visible (the reference arm and --dry-run need no device)."""
+    if args.impl == "ours" and not args.dry_run:
+        import torch
+
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) visible; refusing to run fewer ranks")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__), *sys.argv[1:]]
+    print(f"bench.py: starting {args.gpus} ranks: {' '.join(cmd)}", file=sys.stderr, flush=True)
+    return subprocess.run(cmd).returncode
+
+
+def run_dry(args):
+    """--dry-run: the multi-rank plumbing without a GPU — every rank joins a gloo group on CPU, takes its row band of
+    the config's lattice (sharded.row_bands, as --shard does) or its own map seed (weak mode), and the ranks all-reduce
+    the number of lattice rows they own.  Rank 0 prints one JSON line.  No kernel runs and no throughput is reported."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1406_0559_b200 import sharded
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    os.environ.setdefault("MASTER_PORT", "29531")
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = fields.CONFIGS[args.config]
+    import math
+
+    a1, a2 = cfg.half_widths  # DESIGN.md reading S2: n = 2 ceil(a/d - 1e-9) rays per axis
+    n1, n2 = (2 * math.ceil(a / cfg.ray_spacing - 1e-9) for a in (a1, a2))
+    band = sharded.row_bands(n2, world)[rank] if args.shard else (0, n2)
+    rows = torch.tensor([band[1], 1], dtype=torch.int64)
+    dist.all_reduce(rows, op=dist.ReduceOp.SUM)
+    gathered = [None] * world
+    dist.all_gather_object(gathered, {"rank": rank, "band": list(band), "seed": cfg.seed + (0 if args.shard else rank)})
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "backend": "gloo", "n_gpus": world, "ranks_joined": int(rows[1]),
+                          "scaling": "strong" if args.shard else "weak", "lattice": [n1, n2], "rows_total": int(rows[0]),
+                          "ranks": gathered}), flush=True)
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -625,8 +696,18 @@ def main():
     ap.add_argument("--convolve", action="store_true", help="profile mode: time mlens_convolve on a map of the config's size")
     ap.add_argument("--ablations", action="store_true", help="block mode: load libmlens_ablations.so (kernel / loop variants)")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
+    ap.add_argument("--dry-run", action="store_true", help="N ranks on CPU over gloo: rank start-up, band plan, one all-reduce; no kernels")
     args = ap.parse_args()
-    if args.corun:
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        raise SystemExit(launch_ranks(args))  # N ranks of this command line; rank 0 prints the line
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world_env} ranks")
+    if args.dry_run:
+        run_dry(args)
+    elif args.corun:
         run_corun(args)
     elif args.mpd:
         run_mpd(args)

@@ -8,10 +8,11 @@ import sys
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _run(env_extra):
-    env = dict(os.environ, **env_extra)
+def _run(env_extra, extra_args=()):
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env.update(env_extra)
     return subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "1", "--steps", "1",
-                           "--warmup", "0"], capture_output=True, text=True, env=env, timeout=300)
+                           "--warmup", "0", *extra_args], capture_output=True, text=True, env=env, timeout=600)
 
 
 def test_reference_arm_prints_one_contract_line():
@@ -30,8 +31,50 @@ def test_reference_arm_prints_one_contract_line():
 
 
 def test_reference_arm_other_ranks_are_silent():
-    r = _run({"RANK": "1", "WORLD_SIZE": "2"})
+    r = _run({"RANK": "1", "WORLD_SIZE": "2"}, ["--gpus", "2"])
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_n_starts_n_ranks_itself():
+    # `python bench.py --gpus 2` with no launcher environment: bench.py must start two ranks (torch.distributed.run on
+    # 127.0.0.1), rank 0 prints the one line with n_gpus = 2, rank 1 reports in on stderr.  The reference arm needs no GPU.
+    r = _run({}, ["--gpus", "2"])
+    assert r.returncode == 0, r.stderr
+    assert "starting 2 ranks" in r.stderr and "--nproc-per-node=2" in r.stderr
+    assert "rank 1 of 2: idle" in r.stderr
+    lines = [l for l in r.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
+    assert d["cpu_baseline"]["cores"] == len(os.sched_getaffinity(0))  # not the launcher's OMP_NUM_THREADS=1
+
+
+def test_gpus_n_dry_run_of_the_sharded_launch_over_gloo():
+    # the --shard plumbing without a GPU: two ranks join a gloo group, take their row bands, all-reduce once
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--shard", "--dry-run", "--config", "3"],
+                       capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode == 0, r.stderr
+    lines = [l for l in r.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["dry_run"] is True and d["n_gpus"] == 2 and d["ranks_joined"] == 2 and d["scaling"] == "strong"
+    assert d["lattice"] == [196608, 49152] and d["rows_total"] == 49152
+    bands = [tuple(x["band"]) for x in sorted(d["ranks"], key=lambda x: x["rank"])]
+    assert bands == [(0, 24576), (24576, 24576)]
+
+
+def test_gpus_n_never_falls_back_to_fewer_ranks():
+    # a launcher that started a different number of ranks than --gpus says: refuse
+    r = _run({"RANK": "0", "WORLD_SIZE": "1"}, ["--gpus", "2"])
+    assert r.returncode != 0 and "WORLD_SIZE=1" in r.stderr
+    import torch
+
+    if not torch.cuda.is_available():  # the GPU arm with no (or too few) devices: refuse, do not run one rank
+        env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "1"], capture_output=True,
+                           text=True, env=env, timeout=300)
+        assert r.returncode != 0 and "refusing to run fewer ranks" in r.stderr and r.stdout.strip() == ""
 
 
 def test_gpu_arm_line_contract_from_measured_numbers():
