@@ -291,9 +291,10 @@ long long oracle_index_map(const int* count, long long n_pixels, int* values, in
 // Minimal-bit-width storage (Table B.6).  Bit by bit, straight from the definition: bit k of value q
 // is bit q*bits + k of the stream, and bit i of the stream is bit i%32 of 32-bit word i/32.
 int oracle_bits_needed(unsigned long long max_value) {
-    int b = 1;
-    while (b < 64 && (max_value >> b) != 0ull) ++b;
-    return b;
+    // the number of binary digits of max_value (halve until nothing is left); zero still takes one bit
+    int digits = 0;
+    for (unsigned long long v = max_value; v != 0ull; v /= 2ull) ++digits;
+    return digits > 0 ? digits : 1;
 }
 
 void oracle_pack_bits(const unsigned int* values, long long n, int bits, unsigned int* packed, long long n_words) {
@@ -321,13 +322,15 @@ void oracle_unpack_bits(const unsigned int* packed, long long n, int bits, unsig
 // value at a time.
 void oracle_mpd_rebin(const unsigned long long* hist, int n_bins, double n_avg, double n_pixels, int n_out, double mu_min,
                       double mu_max, double* prob) {
-    for (int k = 0; k < n_out; ++k) prob[k] = 0.0;
+    // reading S20: prob[k] = (number of pixels whose mu falls in bin k) / n_pixels — count the pixels, divide once
+    std::vector<unsigned long long> pixels((size_t)n_out, 0ull);
     const double log_min = std::log10(mu_min), width = (std::log10(mu_max) - log_min) / n_out;
     for (int c = 1; c < n_bins; ++c) {
         if (!hist[c]) continue;
         const double t = (std::log10((double)c / n_avg) - log_min) / width;
-        if (t >= 0.0 && t < (double)n_out) prob[(int)t] += (double)hist[c] / n_pixels;
+        if (t >= 0.0 && t < (double)n_out) pixels[(size_t)(int)t] += hist[c];
     }
+    for (int k = 0; k < n_out; ++k) prob[k] = (double)pixels[(size_t)k] / n_pixels;
 }
 
 int oracle_max_threads(void) {

@@ -171,8 +171,21 @@ def test_mpd_rebin_matches_the_oracle(oracle):
         for n_out, lo, hi in ((100, 0.1, 100.0), (400, 0.05, 300.0), (1, 0.5, 2.0), (7, 1.0, 3.0)):
             prob = h.mpd_rebin(hist, n_out, lo, hi).cpu().numpy()
             ref = oracle.mpd_rebin(hist_ref, h.geometry.n_avg, cfg.npix**2, n_out, lo, hi)
-            assert np.abs(prob - ref).max() <= 1e-12 and abs(prob.sum() - ref.sum()) <= 1e-12
+            assert np.array_equal(prob, ref)  # integer pixel counts per bin, one division: bit-exact and deterministic
+            assert np.array_equal(h.mpd_rebin(hist, n_out, lo, hi).cpu().numpy(), prob)
             assert prob.sum() <= 1.0 + 1e-12
+        # counts that sit EXACTLY on bin edges (N_avg = 36: c = 36, 360, 3600 are mu = 1, 10, 100): mu on an inner edge goes
+        # to the upper bin, mu = mu_min is inside, mu = mu_max is outside — same side as the oracle in every case
+        edge = np.zeros(4000, np.uint64)
+        edge[[35, 36, 37, 359, 360, 361, 3599, 3600, 3601]] = [1, 2, 4, 8, 16, 32, 64, 128, 256]
+        edge_dev = torch.from_numpy(edge.view(np.int64)).cuda()
+        assert h.geometry.n_avg == 36.0
+        for n_out, lo, hi in ((3, 0.1, 100.0), (2, 1.0, 100.0), (4, 1.0, 100.0), (400, 1.0, 10.0), (1, 10.0, 100.0), (6, 0.01, 10000.0)):
+            prob = h.mpd_rebin(edge_dev, n_out, lo, hi).cpu().numpy()
+            ref = oracle.mpd_rebin(edge, 36.0, cfg.npix**2, n_out, lo, hi)
+            assert np.array_equal(prob, ref), (n_out, lo, hi)
+        prob = h.mpd_rebin(edge_dev, 2, 1.0, 100.0).cpu().numpy() * cfg.npix**2  # [1,10) and [10,100)
+        assert prob.tolist() == [2 + 4 + 8, 16 + 32 + 64]
         for bad in ((0, 0.1, 10.0), (401, 0.1, 10.0), (100, 0.0, 10.0), (100, 2.0, 1.0)):
             with pytest.raises(mlens.MlensError):
                 h.mpd_rebin(hist, *bad)
