@@ -432,68 +432,6 @@ def run_block(args):
                       "rays_in_map_frac": st["rays_in_map"] / max(1, st["rays_total"])}), flush=True)
 
 
-def run_corun(args):
-    """--corun S: can the tensor-pipe kernel and the production kernel share the SMs to advantage?  (row f4.)
-    On the centred S x S block: the slim tensor-pipe kernel ("kernel" 5 of the ablations library: 288 threads x 112
-    registers, 1 CTA per SM) shoots the upper quarter on one stream while one CTA per SM of a CUDA-core variant that fits
-    beside it (8 rays per thread, 32-wide tiles: 256 threads x 80 registers) shoots the next quarter on another; each is
-    also timed alone, and the full production kernel shoots both quarters as the yardstick."""
-    import torch
-
-    from paper_1406_0559_b200 import mlens
-
-    torch.cuda.set_device(0)
-    cfg = fields.CONFIGS[args.config]
-    xy, m = fields.lens_field(cfg)
-    S = args.corun
-    hT = mlens.Mlens.from_config(cfg, xy, m, ablations=True)
-    hT.set_option("kernel", 5)
-    hC = mlens.Mlens.from_config(cfg, xy, m, ablations=True)
-    for k, v in (("rays_per_thread", 8), ("tile_x", 32), ("shared_pairs", 0), ("ctas_per_sm", 1)):
-        hC.set_option(k, v)
-    hP = mlens.Mlens.from_config(cfg, xy, m, ablations=True)
-    g = hP.geometry
-    i0, j0, q = (g.n1 - S) // 2, (g.n2 - S) // 2, S // 4
-    cnt = torch.zeros((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
-    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
-
-    def timed(fn):
-        best = None
-        for _ in range(max(2, args.steps)):
-            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-            torch.cuda.synchronize()
-            ev[0].record(); s1.wait_event(ev[0]); s2.wait_event(ev[0])
-            fn(ev)
-            torch.cuda.synchronize()
-            t = [ev[0].elapsed_time(ev[1]), ev[0].elapsed_time(ev[2])]
-            best = t if best is None or max(t) < max(best) else best
-        return best
-
-    def tensor_alone(ev):
-        hT.shoot_block(i0, j0, S, q, count=cnt, stream=s1); ev[1].record(s1); ev[2].record(s1)
-
-    def cuda_alone(ev):
-        hC.shoot_block(i0, j0 + q, S, q, count=cnt, stream=s2); ev[1].record(s2); ev[2].record(s2)
-
-    def both(ev):
-        hT.shoot_block(i0, j0, S, q, count=cnt, stream=s1); ev[1].record(s1)
-        hC.shoot_block(i0, j0 + q, S, q, count=cnt, stream=s2); ev[2].record(s2)
-
-    def production(ev):
-        hP.shoot_block(i0, j0, S, 2 * q, count=cnt, stream=s1); ev[1].record(s1); ev[2].record(s1)
-
-    inter_q = S * q * max(1, len(m))
-    tT, tC, tB, tP = timed(tensor_alone)[0], timed(cuda_alone)[1], timed(both), timed(production)[0]
-    print(json.dumps({"mode": "corun", "config": args.config, "block": [i0, j0, S, S], "quarter_interactions": inter_q,
-                      "tensor_kernel_alone_ms": tT, "cuda_core_1cta_alone_ms": tC,
-                      "co_run_ms": {"tensor_done": tB[0], "cuda_core_done": tB[1]},
-                      "co_run_interactions_per_s": 2 * inter_q / (max(tB) * 1e-3),
-                      "serial_sum_ms": tT + tC, "production_kernel_both_quarters_ms": tP,
-                      "production_interactions_per_s": 2 * inter_q / (tP * 1e-3)}), flush=True)
-    for h in (hT, hC, hP):
-        h.close()
-
-
 def run_mpd(args):
     """--mpd: K launches of mlens_mpd (row f1: MPD histogram + map means) on the config's shot map; HBM roofline."""
     import torch
@@ -568,6 +506,40 @@ def run_mpd(args):
                                            "pack_gbs": (2 + bits / 8) * cfg.npix**2 / (statistics.median(pms) * 1e-3) / 1e9,
                                            "unpack_gbs": (2 + bits / 8) * cfg.npix**2 / (statistics.median(ums) * 1e-3) / 1e9}}),
           flush=True)
+
+
+def run_survey_mode(args):
+    """--survey: maps per second of the many-maps driver (paper_1406_0559_b200/survey.py, row f3) on ONE GPU: M independent
+    maps of the config's class (seeds differ), with 1, 2 and 4 maps in flight.  Timed region per K: create (H2D lens
+    list) + shoot + Eq. 4 + D2H of both maps into pinned host buffers + destroy, for all M maps; host clock around the
+    batch with a device synchronize on both sides.  The lens fields are generated before the clock starts."""
+    import dataclasses
+
+    import torch
+
+    from paper_1406_0559_b200 import survey
+
+    torch.cuda.set_device(0)
+    cfg0 = fields.CONFIGS[args.config]
+    jobs = [survey.MapJob.from_config(dataclasses.replace(cfg0, seed=cfg0.seed + 17 * k)) for k in range(args.maps)]
+    out_c = [torch.empty((cfg0.npix, cfg0.npix), dtype=torch.int32, pin_memory=True) for _ in jobs]
+    out_m = [torch.empty((cfg0.npix, cfg0.npix), dtype=torch.float32, pin_memory=True) for _ in jobs]
+    inter = None
+    rows = []
+    for k in [int(v) for v in args.streams.split(",")]:
+        best = None
+        for rep in range(max(1, args.warmup) + max(1, args.steps)):  # first repetitions are warm-up
+            r = survey.run_survey(jobs, n_streams=k, out_count=out_c, out_mag=out_m)
+            for j, st, c in zip(jobs, r["stats"], out_c):
+                assert st["rays_in_map"] + st["rays_outside"] + st["rays_lost"] == st["rays_total"]
+                assert int(c.sum(dtype=torch.int64)) == st["rays_in_map"]
+            inter = sum(st["rays_total"] * max(1, len(j.lens_m)) for j, st in zip(jobs, r["stats"]))
+            if rep >= max(1, args.warmup) and (best is None or r["seconds"] < best):
+                best = r["seconds"]
+        rows.append({"streams": k, "seconds": best, "maps_per_s": len(jobs) / best, "interactions_per_s": inter / best})
+    print(json.dumps({"mode": "survey", "config": args.config, "workload": f"{len(jobs)} maps of config {args.config}'s class "
+                      f"({cfg0.npix}^2 px, seeds {cfg0.seed}+17k), one GPU, create + shoot + D2H (count and mag) + destroy per map",
+                      "maps": len(jobs), "d2h_bytes_per_map": 8 * cfg0.npix**2, "rows": rows}), flush=True)
 
 
 def run_convolve(args):
@@ -691,11 +663,13 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--shard", action="store_true", help="N > 1: shoot ONE map in row bands + one all-reduce (strong scaling)")
     ap.add_argument("--block", type=int, default=0, help="profile mode: shoot a centred SxS-ray block K times")
-    ap.add_argument("--corun", type=int, default=0, help="profile mode: tensor-pipe + CUDA-core kernels sharing the SMs on an SxS block")
     ap.add_argument("--mpd", action="store_true", help="profile mode: time mlens_mpd on the config's shot map")
     ap.add_argument("--convolve", action="store_true", help="profile mode: time mlens_convolve on a map of the config's size")
     ap.add_argument("--ablations", action="store_true", help="block mode: load libmlens_ablations.so (kernel / loop variants)")
     ap.add_argument("--option", nargs=2, action="append", metavar=("KEY", "VALUE"), help="mlens_set_option (block mode)")
+    ap.add_argument("--survey", action="store_true", help="profile mode: maps/s of the many-maps driver at 1, 2, 4 maps in flight")
+    ap.add_argument("--maps", type=int, default=32, help="--survey: maps per batch")
+    ap.add_argument("--streams", default="1,2,4", help="--survey: comma-separated numbers of maps in flight")
     ap.add_argument("--dry-run", action="store_true", help="N ranks on CPU over gloo: rank start-up, band plan, one all-reduce; no kernels")
     args = ap.parse_args()
     if args.gpus < 1:
@@ -707,8 +681,8 @@ def main():
         raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world_env} ranks")
     if args.dry_run:
         run_dry(args)
-    elif args.corun:
-        run_corun(args)
+    elif args.survey:
+        run_survey_mode(args)
     elif args.mpd:
         run_mpd(args)
     elif args.convolve:

@@ -26,7 +26,9 @@
  *
  * Concurrency.  Calls on one handle must not be issued concurrently from several host threads.  From ONE thread:
  *   - mlens_shoot_block launches of one handle MAY be issued to different streams and overlap on the device: each
- *     launch owns its tile counter (up to 256 launches in flight), the ray counters and the count map are atomic sums;
+ *     launch owns its tile counter (a ring of 256; launch n + 256 is made to wait, on the device, for launch n — an
+ *     event per slot — so more launches in flight are safe, only no longer concurrent), the ray counters and the count
+ *     map are atomic sums;
  *   - mlens_shoot, mlens_mpd, mlens_index_map, mlens_profile_kernel and mlens_convolve use per-handle scratch (events,
  *     histogram slices, spectra, cuFFT plans): calls of these on one handle must be ordered after one another — issue
  *     them to one stream, or order the streams with events.  Use one handle per stream for concurrent maps.
@@ -265,11 +267,9 @@ int mlens_reset_stats(mlens_t* h, void* cuda_stream);
  * (libmlens_ablations.so, which the tests and profiling runs load; the shipped library returns MLENS_EINVAL for them, so
  * the public ABI cannot select a kernel that misses the parity tolerances):
  *   "kernel"       0 = plain FP64 one-ray-per-thread kernel (plumbing/debug), 2 = plain-form FP32 kernel (does NOT meet
- *                  the parity tolerances: the evidence for the difference form; <= 12000 lenses), 3 = tensor-pipe
- *                  experiment (r^2, Re, Im of every interaction from tcgen05 TF32 MMAs; slower than kernel 1 and NOT
- *                  deterministic: its per-ray partial sums meet in shared-memory float atomics), 4 = the round-1
- *                  production kernel (A/B baseline; its loop variant "shared_rcp" 0..2), 5 = kernel 3 slimmed to 8 consumer
- *                  warps (288 threads) so that it can share an SM with a CUDA-core CTA (bench.py --corun)
+ *                  the parity tolerances: the evidence for the difference form; <= 12000 lenses), 4 = the round-1
+ *                  production kernel (A/B baseline; its loop variant "shared_rcp" 0..2).  (3 and 5 were the tensor-pipe
+ *                  experiment of rounds 1-2: closed negative and removed.)
  *   "rays_per_thread" 8 | 16, "tile_x" 64 | 48 | 32 (8 rays only), "shared_pairs" 0..4: the sweep grid of kernel 1
  * Returns MLENS_EINVAL for an unknown key or value. */
 int mlens_set_option(mlens_t* h, const char* key, long long value);
@@ -277,13 +277,26 @@ int mlens_set_option(mlens_t* h, const char* key, long long value);
 /* Thread-local message for the last failure on this thread ("" if none). */
 const char* mlens_last_error(void);
 
-/* Frees everything mlens_create allocated (never the caller's buffers), after synchronising the handle's device.  NULL
- * is allowed.  Device blocks return to a library-owned memory pool (one per device) that KEEPS them for the next
- * handle, so that creating / shooting / destroying map after map does not pay cudaMalloc / cudaFree each time (cudaFree
- * of a map-sized buffer was measured at up to 1.5 s on the B200 box). */
+/* Releases everything mlens_create and later calls on the handle allocated (never the caller's buffers), after
+ * synchronising the handle's device.  NULL is allowed.
+ * MEMORY RETENTION: the device blocks are NOT returned to the driver.  They go to a library-owned memory pool (one per
+ * device) that KEEPS them for the next handle, so that creating / shooting / destroying map after map does not pay
+ * cudaMalloc / cudaFree each time (cudaFree of a map-sized buffer was measured at up to 1.5 s on the B200 box).  For a
+ * handle that used mlens_shoot_host and mlens_convolve at npix = 10000 that is about 2 GB (two maps, three spectra), and a
+ * program that alternates map sizes accumulates one such set per size.  Other allocators in the process (torch's
+ * caching allocator, cuFFT work areas, NCCL) cannot use that memory until mlens_trim_memory is called.  The library
+ * itself trims the pool and retries once when one of its own allocations fails. */
 void mlens_destroy(mlens_t* h);
 
-/* Hand the blocks cached by destroyed handles on the CURRENT device back to the driver (blocks of live handles stay). */
+/* mlens_destroy for a caller who issued ALL work on this handle to `cuda_stream` (or ordered it before that stream with
+ * events): waits for that stream only, not for the whole device, then releases the handle as mlens_destroy does.  A
+ * survey that runs several maps at once, one handle per stream (maps are produced in batches of
+ * thousands), uses this so that finishing one map does not wait for the maps still running on the other streams.
+ * Work of this handle still running on another, unordered stream is a use-after-free.  NULL handle allowed. */
+void mlens_destroy_on_stream(mlens_t* h, void* cuda_stream);
+
+/* Hand the device blocks cached by destroyed handles on the CURRENT device back to the driver, and free the recycled
+ * pinned host blocks (blocks of live handles stay). */
 int mlens_trim_memory(void);
 
 #ifdef __cplusplus

@@ -265,57 +265,108 @@ __global__ void __launch_bounds__(256) index_decode_kernel(const unsigned short*
 // particular map".  Value q (masked to `bits` bits) occupies bits [q*bits, (q+1)*bits) of a little-endian bit stream
 // held in 32-bit words.  HBM-bound: src bytes in, bits/8 bytes out per value.
 // ---------------------------------------------------------------------------------------------------------------
+//
+// pack: 32 values fill exactly `bits` words, so the bit layout repeats with a period of `bits` words.  A CTA iteration
+// takes K = 256 / bits whole periods; thread t < K*bits owns word r = t % bits of period t / bits FOR THE WHOLE LOOP, so
+// the first value that touches its word, the bit offset inside that value and the number of values it needs are
+// computed once (the one-output-word-per-thread form with a 64-bit division per word ran at 28 % of the copy peak).
 template <typename SrcT>
 __global__ void __launch_bounds__(256) pack_bits_kernel(const SrcT* __restrict__ src, long long n, int bits,
                                                         unsigned int* __restrict__ packed, long long n_words) {
-    const unsigned long long mask = bits >= 32 ? 0xffffffffull : ((1ull << bits) - 1ull);
-    const long long stride = (long long)gridDim.x * 256;
-    for (long long w = (long long)blockIdx.x * 256 + threadIdx.x; w < n_words; w += stride) {  // one output word each
-        const long long bit0 = w << 5;
-        long long q = bit0 / bits;
-        int off = (int)(bit0 - q * bits);  // bits of value q that already went into the previous word
-        unsigned int acc = 0u;
-        int filled = 0;
-        while (filled < 32 && q < n) {
-            const unsigned long long v = (unsigned long long)(unsigned int)src[q] & mask;
-            acc |= (unsigned int)((v >> off) << filled);
-            filled += bits - off;
-            off = 0;
-            ++q;
+    const unsigned int mask = bits >= 32 ? 0xffffffffu : ((1u << bits) - 1u);
+    const int periods = 256 / bits;                 // per CTA iteration (bits <= 32 -> >= 8)
+    const int t = threadIdx.x;
+    if (t >= periods * bits) return;
+    const int r = t % bits, g = t / bits;           // word r of period g
+    const int q_in = (32 * r) / bits;               // first value of the period that has bits in word r
+    const int off = 32 * r - q_in * bits;           // bits of that value that went into word r - 1
+    const int n_vals = (off + 31) / bits + 1;       // values with bits in word r (the last may not exist at a ragged end)
+    const long long words_per_iter = (long long)periods * bits, vals_per_iter = (long long)periods * 32;
+    long long w = (long long)blockIdx.x * words_per_iter + t;
+    long long q0 = (long long)blockIdx.x * vals_per_iter + (long long)g * 32 + q_in;
+    for (; w < n_words; w += (long long)gridDim.x * words_per_iter, q0 += (long long)gridDim.x * vals_per_iter) {
+        unsigned long long acc = 0ull;              // value k sits at bit k*bits of acc; word r starts at bit `off`
+        if (q0 + n_vals <= n) {
+#pragma unroll 4
+            for (int k = 0; k < n_vals; ++k)
+                acc |= (unsigned long long)((unsigned int)src[q0 + k] & mask) << (k * bits);
+        } else {
+            for (int k = 0; k < n_vals && q0 + k < n; ++k)
+                acc |= (unsigned long long)((unsigned int)src[q0 + k] & mask) << (k * bits);
         }
-        packed[w] = acc;
+        packed[w] = (unsigned int)(acc >> off);
     }
 }
 
+// unpack: 16 bytes of output per thread (4 int32 or 8 uint16 values) from a two-word window per value; the words of
+// neighbouring values and threads overlap and are served by L1.
 template <typename DstT>
 __global__ void __launch_bounds__(256) unpack_bits_kernel(const unsigned int* __restrict__ packed, long long n, int bits,
                                                           DstT* __restrict__ dst) {
+    constexpr int kPer = 16 / (int)sizeof(DstT);
     const unsigned long long mask = bits >= 32 ? 0xffffffffull : ((1ull << bits) - 1ull);
-    const long long stride = (long long)gridDim.x * 256;
-    for (long long q = (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride) {
+    const long long stride = (long long)gridDim.x * 256, n_vec = n / kPer;
+    auto value = [&](long long q) {
         const long long bit0 = q * bits;
         const long long w = bit0 >> 5;
         const int sh = (int)(bit0 & 31);
         unsigned long long window = (unsigned long long)__ldg(packed + w);
         if (sh + bits > 32) window |= (unsigned long long)__ldg(packed + w + 1) << 32;
-        dst[q] = (DstT)((window >> sh) & mask);
+        return (DstT)((window >> sh) & mask);
+    };
+    for (long long v = (long long)blockIdx.x * 256 + threadIdx.x; v < n_vec; v += stride) {
+        alignas(16) DstT out[kPer];
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) out[k] = value(v * kPer + k);
+        reinterpret_cast<uint4*>(dst)[v] = *reinterpret_cast<const uint4*>(out);
     }
+    for (long long q = n_vec * kPer + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride) dst[q] = value(q);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // Re-binned view of the MPD (the tools bin mpd.dat "into a histogram before they are returned ... By
 // default, the number of bins is set to 100, with a maximum limit of 400").  Reading S20: n_out bins of
 // equal width in log10(mu) on [mu_min, mu_max), mu = count/N_avg; out[k] = (pixels whose mu falls in bin k)/n_pixels;
-// count 0 (mu = 0) and magnifications outside the range are left out.  One thread per exact-histogram bin.
+// count 0 (mu = 0) and magnifications outside the range are left out.
+//
+// Integer-exact and deterministic: the bin of a count value is monotone in the count, so the host turns the n_out + 1
+// bin boundaries into the smallest COUNT of each bin (RebinEdges, found by bisection on the FP64 expression of reading
+// S20 — mlens.cu) and the device only compares integers, adds 64-bit pixel counts (order-independent) and divides each
+// bin once.  The out array is used as 64-bit integer storage until mpd_rebin_finish_kernel converts it in place.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) mpd_rebin_kernel(const unsigned long long* __restrict__ hist, int n_bins, double n_avg,
-                                                        double n_pixels, int n_out, double log_min, double inv_width,
-                                                        double* __restrict__ out) {
-    for (int c = 1 + blockIdx.x * 256 + threadIdx.x; c < n_bins; c += gridDim.x * 256) {
-        const unsigned long long hcount = hist[c];
-        if (hcount == 0ull) continue;
-        const double t = (log10((double)c / n_avg) - log_min) * inv_width;
-        if (t >= 0.0 && t < (double)n_out) atomicAdd(out + (int)t, (double)hcount / n_pixels);
+constexpr int kRebinMaxOut = 400;
+struct RebinEdges {
+    int lo[kRebinMaxOut + 1];  // lo[k] = smallest count whose bin index is >= k, k = 0..n_out (n_bins if there is none)
+};
+
+__global__ void __launch_bounds__(256) mpd_rebin_kernel(const unsigned long long* __restrict__ hist, int n_bins, int n_out,
+                                                        const RebinEdges edges, unsigned long long* __restrict__ out_pixels) {
+    __shared__ unsigned long long acc[kRebinMaxOut];
+    __shared__ int lo[kRebinMaxOut + 1];
+    for (int k = threadIdx.x; k <= n_out; k += 256) lo[k] = edges.lo[k];
+    for (int k = threadIdx.x; k < n_out; k += 256) acc[k] = 0ull;
+    __syncthreads();
+    const int first = lo[0], last = lo[n_out];  // counts in [first, last) have a bin
+    for (long long c = (long long)first + (long long)blockIdx.x * 256 + threadIdx.x; c < n_bins && c < last; c += (long long)gridDim.x * 256) {
+        const unsigned long long pixels = hist[c];
+        if (pixels == 0ull) continue;
+        int a = 0, b = n_out;  // largest k with lo[k] <= c
+        while (b - a > 1) {
+            const int mid = (a + b) >> 1;
+            if (lo[mid] <= (int)c) a = mid; else b = mid;
+        }
+        atomicAdd(&acc[a], pixels);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < n_out; k += 256)
+        if (acc[k]) atomicAdd(&out_pixels[k], acc[k]);
+}
+
+__global__ void __launch_bounds__(512) mpd_rebin_finish_kernel(double* __restrict__ out, int n_out, double n_pixels) {
+    const int k = threadIdx.x;
+    if (k < n_out) {
+        const unsigned long long pixels = reinterpret_cast<const unsigned long long*>(out)[k];
+        out[k] = (double)pixels / n_pixels;
     }
 }
 

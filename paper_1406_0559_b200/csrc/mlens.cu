@@ -20,7 +20,6 @@
 #include "shoot_kernel.cuh"
 #ifdef MLENS_ABLATIONS
 #include "shoot_ablation_kernels.cuh"
-#include "shoot_umma_kernel.cuh"
 #endif
 
 namespace {
@@ -85,6 +84,13 @@ template <typename T>
 cudaError_t dev_alloc(T** p, size_t bytes) {
     if (DevPool* dp = device_pool()) {
         cudaError_t e = cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes, dp->pool, dp->stream);
+        if (e == cudaErrorMemoryAllocation) {
+            // the pool keeps the blocks of destroyed handles (of other map sizes, too): give them back and try once more
+            (void)cudaGetLastError();
+            cudaStreamSynchronize(dp->stream);
+            cudaMemPoolTrimTo(dp->pool, 0);
+            e = cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes, dp->pool, dp->stream);
+        }
         if (e == cudaSuccess) e = cudaStreamSynchronize(dp->stream);  // usable from any stream from here on
         return e;
     }
@@ -132,6 +138,7 @@ constexpr int kChunkSingleMax = 3072;  // largest list kept resident as one chun
 constexpr int kProdTileX = MLENS_PROD_TILE_X, kProdRays = MLENS_PROD_RAYS, kProdSharedPairs = MLENS_PROD_SHARED_PAIRS;
 constexpr int kProdCtas = 2;
 constexpr int kTileCtrSlots = 256;     // ring of dynamic tile counters: one per launch in flight (see launch_block)
+static_assert(kTileCtrSlots == 256, "mlens::slot_done holds one event per ring slot");
 
 }  // namespace
 
@@ -150,6 +157,7 @@ struct mlens {
     unsigned long long* counters_dev;  // in_map, outside, lost, total
     unsigned long long* tile_ctr_dev;  // ring of kTileCtrSlots dynamic tile counters; launch number n uses slot n % kTileCtrSlots
     unsigned long long launch_seq;
+    cudaEvent_t slot_done[256];        // per ring slot: recorded after the launch that used it (created on first use)
     int* max_count_dev;
     mlk::MapStatsDev* mapstats_dev;    // scratch of mlens_mpd (lazily allocated)
     mlk::MapStatsDev* mapstats_host;   // pinned mirror
@@ -163,7 +171,6 @@ struct mlens {
     int* idx_lut;
     long long idx_bins_cap;
     int* idx_n_dev;
-    float* umma_A_dev;                 // kernel 3: ray matrix of one tile in UMMA layout (lazily built)
     unsigned int* mpd_partial;         // sm_count x kMpdSmemBinsMax per-CTA histogram slices (lazily allocated)
     unsigned long long* counters_host;  // pinned mirror (4 counters + max_count)
     // host-buffer path
@@ -222,8 +229,23 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     // Every launch gets its OWN dynamic tile counter, zeroed on the launch's stream: launches of one handle issued to
     // different streams may then overlap without stealing or re-zeroing each other's tiles (the ray counters are
     // plain atomic sums and do not care).  A slot is reused after kTileCtrSlots further launches.
-    P.tile_counter = h->tile_ctr_dev + (h->launch_seq++ % kTileCtrSlots);
+    // The launch that used the slot kTileCtrSlots launches ago may still run on ANOTHER stream: this launch's stream first
+    // waits for the event that launch recorded, so a live counter is never re-zeroed (no duplicated tiles).
+    const int slot = (int)(h->launch_seq++ % kTileCtrSlots);
+    P.tile_counter = h->tile_ctr_dev + slot;
+    if (h->slot_done[slot]) MLENS_CUDA(cudaStreamWaitEvent(st, h->slot_done[slot], 0));
     MLENS_CUDA(cudaMemsetAsync(P.tile_counter, 0, sizeof(unsigned long long), st));
+    struct SlotRelease {  // every return path below records "this slot's launch is done" on the launch's stream
+        mlens_t* h; int slot; cudaStream_t st;
+        ~SlotRelease() {
+            if (!h->slot_done[slot] && cudaEventCreateWithFlags(&h->slot_done[slot], cudaEventDisableTiming) != cudaSuccess) {
+                h->slot_done[slot] = nullptr;
+                (void)cudaGetLastError();
+                return;
+            }
+            cudaEventRecord(h->slot_done[slot], st);
+        }
+    } slot_release{h, slot, st};
     P.bin_mode = h->opt_binning;
 
 #ifdef MLENS_ABLATIONS
@@ -233,40 +255,6 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
         const long long cap = (long long)h->sm_count * 16;
         if (blocks > cap) blocks = cap;
         mlk::shoot_fp64_kernel<<<(unsigned)blocks, 256, 0, st>>>(P);
-        MLENS_CUDA(cudaGetLastError());
-        return MLENS_OK;
-    }
-
-    if (h->opt_kernel == 3 || h->opt_kernel == 5) {  // experimental: pre-reciprocal terms from the tensor pipe (shoot_umma_kernel.cuh)
-        if (!h->umma_A_dev) {
-            std::vector<float> A((size_t)mlk::kUmBlocks * mlk::kUmRays * 8, 0.f);
-            auto tf32 = [](float x) { uint32_t b; memcpy(&b, &x, 4); b = (b + 0x1000u) & 0xffffe000u; memcpy(&x, &b, 4); return x; };
-            for (int rb = 0; rb < mlk::kUmBlocks; ++rb)
-                for (int r = 0; r < mlk::kUmRays; ++r) {
-                    const double dx = (r % mlk::kTile) - 31.5, dy = (2 * rb + r / mlk::kTile) - 31.5;
-                    const double q = (dx * dx + dy * dy) * h->d * h->d;
-                    const float qh = tf32((float)q), ql = tf32((float)(q - (double)qh));
-                    const float row[8] = {1.f, 1.f, (float)dx, (float)dx, (float)dy, (float)dy, qh, ql};
-                    for (int k = 0; k < 8; ++k)
-                        A[((size_t)rb * mlk::kUmABlockBytes + mlk::umma_off_bytes(r, k)) / 4] = row[k];
-                }
-            MLENS_CUDA(dev_alloc(&h->umma_A_dev, A.size() * sizeof(float)));
-            MLENS_CUDA(cudaMemcpy(h->umma_A_dev, A.data(), A.size() * sizeof(float), cudaMemcpyHostToDevice));
-        }
-        P.umma_A = h->umma_A_dev;
-        // kernel 3: 16 consumer warps, 512-lens super-chunks; kernel 5: the slim variant (8 consumer warps, 256-lens
-        // super-chunks: 288 threads x 96 registers, 186 KB) that can share an SM with one CTA of the production kernel
-        const bool slim = h->opt_kernel == 5;
-        const int super = slim ? 256 : 512, cons = slim ? 8 : 16;
-        const size_t smem = (size_t)mlk::kUmBlocks * mlk::kUmABlockBytes + (size_t)(super / mlk::kUmLenses) * mlk::kUmChunkBytes +
-                            (size_t)mlk::kTile * mlk::kTile * sizeof(float2) + sizeof(mlk::UmmaShared) + 1024;
-        const long long n_tiles = (long long)P.tiles_x * P.tiles_y;
-        long long grid = h->sm_count;
-        if (grid > n_tiles) grid = n_tiles;
-        void (*uk)(const mlk::ShootParams) = slim ? mlk::shoot_umma_kernel<8, 256> : mlk::shoot_umma_kernel<16, 512>;
-        MLENS_CUDA(cudaFuncSetAttribute(uk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        MLENS_CUDA(cudaFuncSetAttribute(uk, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
-        uk<<<(unsigned)grid, 32 * (cons + 1), smem, st>>>(P);
         MLENS_CUDA(cudaGetLastError());
         return MLENS_OK;
     }
@@ -456,11 +444,17 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
 
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = dev_alloc(&h->lens_dev, sizeof(float4) * (size_t)(n_lens > 0 ? n_lens : 1));
+    // The blocks are recycled ones (they hold a previous handle's lens list and counters) and the shooting streams are
+    // not ordered with the legacy default stream: initialise them on the pool's own stream and wait for it, so that the
+    // handle is complete before any stream can use it.
+    DevPool* dp = device_pool();
+    cudaStream_t init_st = dp ? dp->stream : (cudaStream_t)0;
     if (e == cudaSuccess && n_lens > 0)
-        e = cudaMemcpy(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice);
+        e = cudaMemcpyAsync(h->lens_dev, packed.data(), sizeof(float4) * (size_t)n_lens, cudaMemcpyHostToDevice, init_st);
     // one block for the small device state: 8 ray counters, the ring of tile counters, max_count
     if (e == cudaSuccess) e = dev_alloc(&h->counters_dev, (8 + kTileCtrSlots + 1) * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(h->counters_dev, 0, (8 + kTileCtrSlots + 1) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->counters_dev, 0, (8 + kTileCtrSlots + 1) * sizeof(unsigned long long), init_st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(init_st);
     if (e == cudaSuccess) {
         h->tile_ctr_dev = h->counters_dev + 8;
         h->max_count_dev = reinterpret_cast<int*>(h->counters_dev + 8 + kTileCtrSlots);
@@ -479,20 +473,30 @@ int mlens_create(mlens_t** out, double kappa, double gamma, double s, double map
     return MLENS_OK;
 }
 
-void mlens_destroy(mlens_t* h) {
+namespace {
+// device_wide: wait for every stream of the device (the handle may have been used on any of them); otherwise only for `st`
+void destroy_impl(mlens_t* h, bool device_wide, cudaStream_t st);
+}
+
+void mlens_destroy(mlens_t* h) { destroy_impl(h, true, nullptr); }
+
+void mlens_destroy_on_stream(mlens_t* h, void* cuda_stream) { destroy_impl(h, false, (cudaStream_t)cuda_stream); }
+
+namespace {
+void destroy_impl(mlens_t* h, bool device_wide, cudaStream_t st) {
     if (!h) return;
     // the handle's blocks go back to ITS device's pool: make that device current for the duration, and let every kernel
     // that may still use them finish first (what cudaFree used to do implicitly)
     int cur = -1;
     cudaGetDevice(&cur);
     if (cur != h->device) cudaSetDevice(h->device);
-    cudaDeviceSynchronize();
+    if (device_wide) cudaDeviceSynchronize();
+    else cudaStreamSynchronize(st);
     dev_free(h->lens_dev);
     dev_free(h->counters_dev);  // also holds the tile counters and max_count
     dev_free(h->mapstats_dev);
     pinned_free(h->mapstats_host);
     dev_free(h->mpd_partial);
-    dev_free(h->umma_A_dev);
     dev_free(h->idx_hist);
     dev_free(h->idx_lut);
     dev_free(h->idx_n_dev);
@@ -505,6 +509,8 @@ void mlens_destroy(mlens_t* h) {
     dev_free(h->count_own);
     dev_free(h->mag_own);
     if (h->own_stream) cudaStreamDestroy(h->own_stream);
+    for (cudaEvent_t ev : h->slot_done)
+        if (ev) cudaEventDestroy(ev);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     if (h->evk0) cudaEventDestroy(h->evk0);
@@ -512,12 +518,19 @@ void mlens_destroy(mlens_t* h) {
     if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
     delete h;
 }
+}  // namespace
 
 int mlens_trim_memory(void) {
     if (DevPool* dp = device_pool()) {
         MLENS_CUDA(cudaStreamSynchronize(dp->stream));
         MLENS_CUDA(cudaMemPoolTrimTo(dp->pool, 0));
     }
+    std::vector<void*> pinned;
+    {
+        std::lock_guard<std::mutex> lock(g_pool_mutex);
+        pinned.swap(g_pinned_free);
+    }
+    for (void* p : pinned) cudaFreeHost(p);
     return MLENS_OK;
 }
 
@@ -538,7 +551,7 @@ int mlens_set_option(mlens_t* h, const char* key, long long value) {
         return fail(MLENS_EINVAL, "option %s=%lld needs the MLENS_ABLATIONS build of the library", key, value);
 #endif
     if (!strcmp(key, "kernel")) {
-        if (value < 0 || value > 5) return fail(MLENS_EINVAL, "kernel must be 0..5");
+        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(MLENS_EINVAL, "kernel must be 0, 1, 2 or 4");
         h->opt_kernel = (int)value;
     } else if (!strcmp(key, "tile_x")) {
         if (value != 64 && value != 48 && value != 32) return fail(MLENS_EINVAL, "tile_x must be 64, 48 or 32");
@@ -707,8 +720,10 @@ int mlens_pack_map(mlens_t* h, const void* src_dev, int src_bits, int bits, unsi
     if (src_bits != 16 && src_bits != 32) return fail(MLENS_EINVAL, "src_bits must be 16 or 32");
     if (bits < 1 || bits > src_bits) return fail(MLENS_EINVAL, "bits must be 1..src_bits");
     const long long n = (long long)h->npix * h->npix, n_words = mlens_packed_words(n, bits);
-    long long blocks = (n_words + 255) / 256;
+    const long long words_per_cta = (long long)(256 / bits) * bits;  // whole 32-value periods per CTA iteration
+    long long blocks = (n_words + words_per_cta - 1) / words_per_cta;
     if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
+    if (blocks < 1) blocks = 1;
     if (src_bits == 32)
         mlk::pack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const int*)src_dev, n, bits, packed_dev, n_words);
     else
@@ -723,8 +738,9 @@ int mlens_unpack_map(mlens_t* h, const unsigned int* packed_dev, int bits, void*
     if (dst_bits != 16 && dst_bits != 32) return fail(MLENS_EINVAL, "dst_bits must be 16 or 32");
     if (bits < 1 || bits > dst_bits) return fail(MLENS_EINVAL, "bits must be 1..dst_bits");
     const long long n = (long long)h->npix * h->npix;
-    long long blocks = (n + 255) / 256;
+    long long blocks = (n / (dst_bits == 32 ? 4 : 8) + 255) / 256;  // 16 bytes of output per thread
     if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
+    if (blocks < 1) blocks = 1;
     if (dst_bits == 32)
         mlk::unpack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (int*)dst_dev);
     else
@@ -742,12 +758,26 @@ int mlens_mpd_rebin(mlens_t* h, const unsigned long long* hist_dev, int n_bins, 
     if (!std::isfinite(mu_min) || !std::isfinite(mu_max) || !(mu_min > 0) || !(mu_max > mu_min))
         return fail(MLENS_EINVAL, "0 < mu_min < mu_max required");
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    MLENS_CUDA(cudaMemsetAsync(prob_dev, 0, sizeof(double) * (size_t)n_out, st));
-    const double log_min = std::log10(mu_min), inv_width = (double)n_out / (std::log10(mu_max) - log_min);
-    int blocks = (n_bins + 255) / 256;
-    if (blocks > h->sm_count * 8) blocks = h->sm_count * 8;
-    mlk::mpd_rebin_kernel<<<blocks, 256, 0, st>>>(hist_dev, n_bins, h->geo.n_avg, (double)h->npix * (double)h->npix, n_out, log_min,
-                                                   inv_width, prob_dev);
+    MLENS_CUDA(cudaMemsetAsync(prob_dev, 0, sizeof(double) * (size_t)n_out, st));  // 64-bit integer zeros, too
+    // Reading S20: bin(c) = floor((log10(c / N_avg) - log10(mu_min)) / width), width = (log10(mu_max) - log10(mu_min)) / n_out,
+    // kept when 0 <= bin < n_out.  The expression is monotone in c, so each bin is a range of counts: find the first count of
+    // every bin here, by bisection on that very expression, and let the device work on integers only.
+    const double log_min = std::log10(mu_min), width = (std::log10(mu_max) - log_min) / n_out, n_avg = h->geo.n_avg;
+    auto position = [&](long long c) { return (std::log10((double)c / n_avg) - log_min) / width; };
+    mlk::RebinEdges edges;
+    for (int k = 0; k <= n_out; ++k) {
+        long long a = 0, b = n_bins;  // position(a) < k (or a = 0: no logarithm), position(b) >= k (or b = n_bins: none)
+        while (b - a > 1) {
+            const long long mid = a + (b - a) / 2;
+            if (position(mid) >= (double)k) b = mid; else a = mid;
+        }
+        edges.lo[k] = (int)b;
+    }
+    long long blocks = ((long long)n_bins + 255) / 256;
+    if (blocks > (long long)h->sm_count * 8) blocks = (long long)h->sm_count * 8;
+    mlk::mpd_rebin_kernel<<<(unsigned)blocks, 256, 0, st>>>(hist_dev, n_bins, n_out, edges, reinterpret_cast<unsigned long long*>(prob_dev));
+    MLENS_CUDA(cudaGetLastError());
+    mlk::mpd_rebin_finish_kernel<<<1, 512, 0, st>>>(prob_dev, n_out, (double)h->npix * (double)h->npix);
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }

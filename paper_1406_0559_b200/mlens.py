@@ -90,6 +90,8 @@ def lib(ablations: bool = False) -> ctypes.CDLL:
     L.mlens_trim_memory.restype = ci
     L.mlens_destroy.argtypes = [vp]
     L.mlens_destroy.restype = None
+    L.mlens_destroy_on_stream.argtypes = [vp, vp]
+    L.mlens_destroy_on_stream.restype = None
     for name in ("mlens_create", "mlens_shoot", "mlens_shoot_block", "mlens_shoot_host", "mlens_magnification", "mlens_mpd",
                  "mlens_profile_kernel", "mlens_convolve", "mlens_index_map", "mlens_unindex_map",
                  "mlens_get_geometry", "mlens_get_stats", "mlens_reset_stats", "mlens_set_option", "mlens_bits_needed",
@@ -167,9 +169,14 @@ class Mlens:
     def _ck(self, rc: int):
         _check(rc, self._L)
 
-    def close(self):
+    def close(self, stream=None):
+        """mlens_destroy; with ``stream``: mlens_destroy_on_stream — waits for that stream only (every call on this handle
+        must have been issued to it), so maps running on other streams are not waited for."""
         if getattr(self, "_h", None) is not None and self._h:
-            self._L.mlens_destroy(self._h)
+            if stream is None:
+                self._L.mlens_destroy(self._h)
+            else:
+                self._L.mlens_destroy_on_stream(self._h, _stream_ptr(stream))
             self._h = ctypes.c_void_p()
 
     def __del__(self):
@@ -301,6 +308,9 @@ class Mlens:
 
         dtype = dtype or torch.int32
         assert packed.is_cuda and packed.is_contiguous() and packed.dtype == torch.int32 and dtype in (torch.int32, torch.uint16)
+        n_words = int(self._L.mlens_packed_words(self.npix**2, int(bits)))
+        if n_words < 0 or packed.numel() < n_words:  # a short buffer would be read out of bounds on the device
+            raise MlensError(EINVAL, f"packed holds {packed.numel()} words, a {self.npix}^2 map at {bits} bits needs {n_words}")
         dst = torch.empty((self.npix, self.npix), dtype=dtype, device="cuda")
         self._ck(self._L.mlens_unpack_map(self._h, ctypes.c_void_p(packed.data_ptr()), int(bits), ctypes.c_void_p(dst.data_ptr()),
                                           32 if dtype == torch.int32 else 16, _stream_ptr(stream)))
@@ -310,7 +320,7 @@ class Mlens:
         """mlens_mpd_rebin: the exact MPD histogram -> n_out (<= 400) bins of equal width in log10(mu); float64 [n_out]."""
         import torch
 
-        assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous()
+        assert hist.is_cuda and hist.dtype == torch.int64 and hist.is_contiguous() and hist.numel() >= 2
         prob = torch.empty((int(n_out),), dtype=torch.float64, device="cuda")
         self._ck(self._L.mlens_mpd_rebin(self._h, ctypes.c_void_p(hist.data_ptr()), int(hist.numel()), int(n_out), float(mu_min),
                                          float(mu_max), ctypes.c_void_p(prob.data_ptr()), _stream_ptr(stream)))

@@ -8,7 +8,7 @@ Not a pytest module (no test_ prefix): run ONE tool per gpurun call, as /opt/ski
 Cases: (a) production shooting kernel, lens list resident as one chunk, every binning route, near-lens list in play;
 (b) the same kernel streaming a 5000-lens list in double-buffered chunks (mbarrier phases, bulk copies); (c) near-list
 overflow -> FP64 fallback; (d) mlens_mpd with more than 48 Ki bins (shared + global bins) and (e) mlens_index_map /
-mlens_unindex_map; (f) the -DMLENS_ABLATIONS kernels (FP64, plain FP32, tensor-pipe experiment, round-1 kernel) if that library is built.
+mlens_unindex_map; (f) the -DMLENS_ABLATIONS kernels (FP64, plain FP32, round-1 kernel) if that library is built.
 Sizes are tiny: the tools slow kernels down by 10-1000x.  Each case checks its result so that a run is also a smoke test.
 The summaries of the runs are kept under profiles/.
 """
@@ -94,14 +94,14 @@ def case_ablation_kernels():
     with mlens.Mlens.from_config(cfg, xy, m, ablations=True) as h:
         g = h.geometry
         blk = (g.n1 // 2 - 64, g.n2 // 2 - 64, 128, 128)
-        for kern in (1, 0, 2, 3, 4):
+        for kern in (1, 0, 2, 4):
             h.set_option("kernel", kern)
             cnt = torch.zeros((cfg.npix, cfg.npix), dtype=torch.int32, device="cuda")
             h.reset_stats()
             h.shoot_block(*blk, count=cnt)
             res[kern] = h.stats()["rays_in_map"]
             assert int(cnt.sum()) == res[kern]
-    return f"kernels 1/0/2/3/4 on a 128x128 block x {len(m)} lenses: in_map {res}"
+    return f"kernels 1/0/2/4 on a 128x128 block x {len(m)} lenses: in_map {res}"
 
 
 if __name__ == "__main__":

@@ -133,3 +133,46 @@ def test_band_decomposition_is_bit_identical_on_gpu():
             assert mag is not None and st["band"][0] % sharded.TILE == 0
         assert tot == st_full["rays_total"] == h.geometry.n1 * h.geometry.n2
         assert torch.equal(acc, full)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# many maps on one GPU (paper_1406_0559_b200/survey.py): the paper's own way of scaling
+# ---------------------------------------------------------------------------------------------------------------
+def test_survey_parameter_grid_builds_the_jobs():
+    from paper_1406_0559_b200 import survey
+
+    base = fields.MapConfig("grid", 64, 4.0, 0.3, 0.1, 0.0, 4, "unit", 900)
+    jobs = survey.parameter_grid(base, [0.3, 0.5], [0.0, 0.2], [0.0, 0.9])
+    assert len(jobs) == 8 and [j.cfg.seed for j in jobs] == list(range(900, 908))
+    assert {(j.cfg.kappa, j.cfg.gamma, j.cfg.s) for j in jobs} == {(k, g, s) for k in (0.3, 0.5) for g in (0.0, 0.2) for s in (0.0, 0.9)}
+    for j in jobs:  # Eq. 3: N* follows kappa_* = (1 - s) kappa of each grid point
+        assert len(j.lens_m) == j.cfg.n_lens and j.lens_xy.shape == (j.cfg.n_lens, 2)
+    if not torch.cuda.is_available():
+        with pytest.raises(RuntimeError):
+            survey.run_survey(jobs[:1])
+
+
+@pytest.mark.gpu
+def test_survey_driver_matches_one_map_at_a_time():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1406_0559_b200 import mlens, survey
+
+    base = fields.MapConfig("grid", 160, 6.0, 0.4, 0.1, 0.0, 4, "salpeter", 910)
+    jobs = survey.parameter_grid(base, [0.35, 0.6], [0.0, 0.15], [0.0, 0.5, 0.9])  # 12 maps, different lattices and N*
+    ref = []
+    for j in jobs:
+        with mlens.Mlens.from_config(j.cfg, j.lens_xy, j.lens_m) as h:
+            c, m, st = h.shoot()
+            ref.append((c.cpu(), m.cpu(), st))
+    for k in (1, 3, 4):
+        r = survey.run_survey(jobs, n_streams=k)
+        assert r["n_streams"] == k and len(r["stats"]) == len(jobs)
+        for (c, m, st), c2, m2, st2 in zip(ref, r["count"], r["mag"], r["stats"]):
+            assert torch.equal(c, c2) and torch.equal(m, m2)  # same kernels, same tiles: bit-identical
+            for key in ("rays_total", "rays_in_map", "rays_outside", "rays_lost", "max_count"):
+                assert st[key] == st2[key], key
+    # caller-owned numpy result buffers, counts only
+    bufs = [np.empty((j.cfg.npix, j.cfg.npix), np.int32) for j in jobs]
+    r = survey.run_survey(jobs, n_streams=2, want_mag=False, out_count=bufs)
+    assert r["mag"] is None and all(np.array_equal(b, c.numpy()) for b, (c, _, _) in zip(bufs, ref))
