@@ -179,7 +179,8 @@ int mlens_mpd_static(const int* count_dev, long long n_pixels, double n_avg, uns
  *   values_dev   DEVICE max_values int32, caller-owned: the index file, distinct counts in ASCENDING order
  *   indexed_dev  DEVICE npix*npix unsigned 16-bit, caller-owned: index of every pixel's count
  *   n_distinct   HOST out: number of distinct values (bits needed = ceil(log2(n_distinct)), PAPER.md Table B.6)
- * Synchronises `cuda_stream` (the distinct count comes back to the host).  Integer-exact and lossless:
+ * Synchronises `cuda_stream` once (the distinct count comes back to the host; a second pass and synchronisation only
+ * if the map's largest count exceeds the histogram capacity the handle has, initially 16 Ki bins).  Integer-exact and lossless:
  * mlens_unindex_map(indexed, values) reproduces count_dev bit for bit.  MLENS_ERANGE if the map has more than 65536
  * distinct values (the paper's maximum over ~70 000 maps is 58 042, Table B.5) or more than max_values; *n_distinct is
  * set in both cases. */

@@ -266,61 +266,97 @@ __global__ void __launch_bounds__(256) index_decode_kernel(const unsigned short*
 // held in 32-bit words.  HBM-bound: src bytes in, bits/8 bytes out per value.
 // ---------------------------------------------------------------------------------------------------------------
 //
-// pack: 32 values fill exactly `bits` words, so the bit layout repeats with a period of `bits` words.  A CTA iteration
-// takes K = 256 / bits whole periods; thread t < K*bits owns word r = t % bits of period t / bits FOR THE WHOLE LOOP, so
-// the first value that touches its word, the bit offset inside that value and the number of values it needs are
-// computed once (the one-output-word-per-thread form with a 64-bit division per word ran at 28 % of the copy peak).
+// pack: 32 values fill exactly `bits` words, so the bit layout repeats with a period of `bits` words.  A CTA takes a
+// chunk of n_sub x K whole periods (K = 256 / bits, about 8192 values): the values come in with coalesced 16-byte loads
+// into shared memory (several per thread in flight), then thread t < K*bits builds word r = t % bits of period t / bits of
+// every one of the n_sub sub-blocks — the first value that touches its word, the bit offset inside that value and the
+// number of values it needs are the same each time and computed once.  (One output word per thread straight from global
+// memory ran at 28 % of the copy peak: a 64-bit division per word and three dependent 2-byte loads per thread in flight.)
+constexpr int kPackChunkValues = 8192;  // upper bound of the values of one chunk (shared memory: 16 KB / 32 KB)
+
 template <typename SrcT>
 __global__ void __launch_bounds__(256) pack_bits_kernel(const SrcT* __restrict__ src, long long n, int bits,
-                                                        unsigned int* __restrict__ packed, long long n_words) {
+                                                        unsigned int* __restrict__ packed, long long n_words, int n_sub) {
+    __shared__ __align__(16) SrcT sv[kPackChunkValues];
     const unsigned int mask = bits >= 32 ? 0xffffffffu : ((1u << bits) - 1u);
-    const int periods = 256 / bits;                 // per CTA iteration (bits <= 32 -> >= 8)
+    const int periods = 256 / bits;                 // per sub-block (bits <= 32 -> >= 8)
+    const int words_per_sub = periods * bits, vals_per_sub = periods * 32;
+    const int chunk_vals = n_sub * vals_per_sub;    // <= kPackChunkValues, a multiple of 32 values (>= 64 bytes)
+    const long long chunk_words = (long long)n_sub * words_per_sub;
     const int t = threadIdx.x;
-    if (t >= periods * bits) return;
-    const int r = t % bits, g = t / bits;           // word r of period g
+    const int r = t % bits, g = t / bits;           // word r of period g of each sub-block
     const int q_in = (32 * r) / bits;               // first value of the period that has bits in word r
     const int off = 32 * r - q_in * bits;           // bits of that value that went into word r - 1
-    const int n_vals = (off + 31) / bits + 1;       // values with bits in word r (the last may not exist at a ragged end)
-    const long long words_per_iter = (long long)periods * bits, vals_per_iter = (long long)periods * 32;
-    long long w = (long long)blockIdx.x * words_per_iter + t;
-    long long q0 = (long long)blockIdx.x * vals_per_iter + (long long)g * 32 + q_in;
-    for (; w < n_words; w += (long long)gridDim.x * words_per_iter, q0 += (long long)gridDim.x * vals_per_iter) {
-        unsigned long long acc = 0ull;              // value k sits at bit k*bits of acc; word r starts at bit `off`
-        if (q0 + n_vals <= n) {
-#pragma unroll 4
-            for (int k = 0; k < n_vals; ++k)
-                acc |= (unsigned long long)((unsigned int)src[q0 + k] & mask) << (k * bits);
-        } else {
-            for (int k = 0; k < n_vals && q0 + k < n; ++k)
-                acc |= (unsigned long long)((unsigned int)src[q0 + k] & mask) << (k * bits);
+    const int n_vals = (off + 31) / bits + 1;       // values with bits in word r (the last may lie beyond a ragged end)
+    constexpr int kVec = 16 / (int)sizeof(SrcT);
+    const unsigned int mask_vec = sizeof(SrcT) == 2 ? (mask & 0xffffu) * 0x10001u : mask;  // two 16-bit lanes per word
+    const long long n_chunks = (n + chunk_vals - 1) / chunk_vals;
+    for (long long c = blockIdx.x; c < n_chunks; c += gridDim.x) {
+        const long long base = c * chunk_vals;
+        __syncthreads();                            // the previous chunk has been consumed
+        if (base + chunk_vals <= n) {               // values are masked to `bits` bits here, 4 or 8 at a time
+            const uint4* gsrc = reinterpret_cast<const uint4*>(src + base);
+            for (int v = t; v < chunk_vals / kVec; v += 256) {
+                uint4 x = __ldg(gsrc + v);
+                x.x &= mask_vec; x.y &= mask_vec; x.z &= mask_vec; x.w &= mask_vec;
+                reinterpret_cast<uint4*>(sv)[v] = x;
+            }
+        } else {                                    // ragged end: zero-filled
+            for (int v = t; v < chunk_vals; v += 256) sv[v] = base + v < n ? (SrcT)((unsigned int)src[base + v] & mask) : (SrcT)0;
         }
-        packed[w] = (unsigned int)(acc >> off);
+        __syncthreads();
+        if (t < words_per_sub) {
+            const SrcT* mine = sv + g * 32 + q_in;
+            long long w = c * chunk_words + t;
+            for (int sub = 0; sub < n_sub && w < n_words; ++sub, w += words_per_sub, mine += vals_per_sub) {
+                // value k starts at bit k*bits - off of the word: the first one loses its low `off` bits to the previous
+                // word, the others are shifted up by less than 32 (they overlap the word) — 32-bit shifts only
+                unsigned int acc = (unsigned int)mine[0] >> off;
+#pragma unroll 4
+                for (int k = 1; k < n_vals; ++k) acc |= (unsigned int)mine[k] << (k * bits - off);
+                packed[w] = acc;
+            }
+        }
     }
 }
 
-// unpack: 16 bytes of output per thread (4 int32 or 8 uint16 values) from a two-word window per value; the words of
-// neighbouring values and threads overlap and are served by L1.
+// unpack: 16 bytes of output per thread (4 int32 or 8 uint16 values).  Their bits span at most five consecutive words:
+// five loads per thread, then the 160-bit window is shifted down by `bits` per value (funnel shifts) — a two-word window
+// per value costs 16 loads per thread and was bound by L1 wavefronts (51 % of the copy peak).
 template <typename DstT>
 __global__ void __launch_bounds__(256) unpack_bits_kernel(const unsigned int* __restrict__ packed, long long n, int bits,
-                                                          DstT* __restrict__ dst) {
+                                                          DstT* __restrict__ dst, long long n_words) {
     constexpr int kPer = 16 / (int)sizeof(DstT);
-    const unsigned long long mask = bits >= 32 ? 0xffffffffull : ((1ull << bits) - 1ull);
+    const unsigned int mask = bits >= 32 ? 0xffffffffu : ((1u << bits) - 1u);
     const long long stride = (long long)gridDim.x * 256, n_vec = n / kPer;
-    auto value = [&](long long q) {
+    for (long long v = (long long)blockIdx.x * 256 + threadIdx.x; v < n_vec; v += stride) {
+        const long long bit0 = v * kPer * bits;
+        const long long w0 = bit0 >> 5;
+        const int sh = (int)(bit0 & 31);
+        unsigned int x0 = __ldg(packed + w0);
+        unsigned int x1 = w0 + 1 < n_words ? __ldg(packed + w0 + 1) : 0u;
+        unsigned int x2 = w0 + 2 < n_words ? __ldg(packed + w0 + 2) : 0u;
+        unsigned int x3 = w0 + 3 < n_words ? __ldg(packed + w0 + 3) : 0u;
+        unsigned int x4 = w0 + 4 < n_words ? __ldg(packed + w0 + 4) : 0u;
+        x0 = __funnelshift_rc(x0, x1, sh); x1 = __funnelshift_rc(x1, x2, sh); x2 = __funnelshift_rc(x2, x3, sh);
+        x3 = __funnelshift_rc(x3, x4, sh); x4 >>= sh;
+        alignas(16) DstT out[kPer];
+#pragma unroll
+        for (int k = 0; k < kPer; ++k) {
+            out[k] = (DstT)(x0 & mask);
+            x0 = __funnelshift_rc(x0, x1, bits); x1 = __funnelshift_rc(x1, x2, bits); x2 = __funnelshift_rc(x2, x3, bits);
+            x3 = __funnelshift_rc(x3, x4, bits); x4 = bits >= 32 ? 0u : x4 >> bits;
+        }
+        reinterpret_cast<uint4*>(dst)[v] = *reinterpret_cast<const uint4*>(out);
+    }
+    for (long long q = n_vec * kPer + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride) {  // < kPer values
         const long long bit0 = q * bits;
         const long long w = bit0 >> 5;
         const int sh = (int)(bit0 & 31);
         unsigned long long window = (unsigned long long)__ldg(packed + w);
         if (sh + bits > 32) window |= (unsigned long long)__ldg(packed + w + 1) << 32;
-        return (DstT)((window >> sh) & mask);
-    };
-    for (long long v = (long long)blockIdx.x * 256 + threadIdx.x; v < n_vec; v += stride) {
-        alignas(16) DstT out[kPer];
-#pragma unroll
-        for (int k = 0; k < kPer; ++k) out[k] = value(v * kPer + k);
-        reinterpret_cast<uint4*>(dst)[v] = *reinterpret_cast<const uint4*>(out);
+        dst[q] = (DstT)((unsigned int)(window >> sh) & mask);
     }
-    for (long long q = n_vec * kPer + (long long)blockIdx.x * 256 + threadIdx.x; q < n; q += stride) dst[q] = value(q);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

@@ -26,6 +26,12 @@ namespace {
 
 thread_local char g_err[512] = "";
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is state of the FUNCTION, not of the launch: two host threads (one
+// handle each, e.g. the workers of survey.py) that set it to different sizes and then launch would race — the launch with
+// the larger request fails with "invalid argument" when the other thread's smaller value is the current one.  Every
+// set-attribute + launch pair of a kernel with dynamic shared memory runs under this mutex (microseconds of host time).
+std::mutex g_launch_mutex;
+
 int fail(int code, const char* fmt, ...) {
     va_list ap;
     va_start(ap, fmt);
@@ -335,6 +341,7 @@ int launch_block(mlens_t* h, long long i0, long long j0, long long ni, long long
     if (h->opt_ctas_per_sm > 0) ctas = h->opt_ctas_per_sm;
     long long grid = (long long)h->sm_count * ctas;
     if (grid > n_tiles) grid = n_tiles;
+    std::lock_guard<std::mutex> launch_lock(g_launch_mutex);
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     MLENS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     kern<<<(unsigned)grid, threads, smem, st>>>(P);
@@ -624,10 +631,13 @@ int mlens_mpd(mlens_t* h, const int* count_dev, unsigned long long* hist_dev, in
     if (blocks > h->sm_count) blocks = h->sm_count;  // one persistent 1024-thread CTA per SM
     if (blocks < 1) blocks = 1;
     const size_t smem = sizeof(unsigned int) * (size_t)smem_bins;
-    MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n, hist_dev, n_bins, smem_bins,
-                                                                       h->mpd_partial, h->mapstats_dev);
-    MLENS_CUDA(cudaGetLastError());
+    {
+        std::lock_guard<std::mutex> launch_lock(g_launch_mutex);
+        MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n, hist_dev, n_bins, smem_bins,
+                                                                           h->mpd_partial, h->mapstats_dev);
+        MLENS_CUDA(cudaGetLastError());
+    }
     mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(h->mpd_partial, (int)blocks, smem_bins, hist_dev, n_bins, h->mapstats_dev);
     MLENS_CUDA(cudaGetLastError());
     if (stats) {
@@ -651,32 +661,38 @@ int mlens_index_map(mlens_t* h, const int* count_dev, int* values_dev, int max_v
     if (max_values < 1) return fail(MLENS_EINVAL, "max_values must be >= 1");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long n = (long long)h->npix * h->npix;
-    // (1) largest count -> number of histogram bins
-    if (int rc = launch_magnification(h, count_dev, nullptr, st)) return rc;
-    MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 4, h->max_count_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
-    MLENS_CUDA(cudaStreamSynchronize(st));
-    int max_count;
-    memcpy(&max_count, h->counters_host + 4, sizeof(int));
-    const long long n_bins = (long long)max_count + 2;
-    if (n_bins > 2147483647LL) return fail(MLENS_ERANGE, "largest count %d: the histogram would need more than 2^31-1 bins", max_count);
-    if (n_bins > h->idx_bins_cap) {
-        dev_free(h->idx_hist);
-        dev_free(h->idx_lut);
-        h->idx_hist = nullptr; h->idx_lut = nullptr; h->idx_bins_cap = 0;
-        MLENS_CUDA(dev_alloc(&h->idx_hist, sizeof(unsigned long long) * (size_t)n_bins));
-        MLENS_CUDA(dev_alloc(&h->idx_lut, sizeof(int) * (size_t)n_bins));
-        h->idx_bins_cap = n_bins;
+    // The histogram needs max(count) + 2 bins, which is not known yet.  Instead of a pass over the map to find it (and a
+    // host round trip), take the capacity the handle already has (at least 16 Ki bins), and let the MPD pass itself say
+    // whether it was enough: its statistics count the pixels clamped into the last bin.  Only then is the histogram
+    // re-made with max_count + 2 bins (the capacity is kept, so the next map of a survey does not pay this again).
+    long long n_bins = h->idx_bins_cap > 0 ? h->idx_bins_cap : 16384;
+    int nd = 0;
+    for (int attempt = 0;; ++attempt) {
+        if (n_bins > h->idx_bins_cap) {
+            dev_free(h->idx_hist);
+            dev_free(h->idx_lut);
+            h->idx_hist = nullptr; h->idx_lut = nullptr; h->idx_bins_cap = 0;
+            MLENS_CUDA(dev_alloc(&h->idx_hist, sizeof(unsigned long long) * (size_t)n_bins));
+            MLENS_CUDA(dev_alloc(&h->idx_lut, sizeof(int) * (size_t)n_bins));
+            h->idx_bins_cap = n_bins;
+        }
+        if (!h->idx_n_dev) MLENS_CUDA(dev_alloc(&h->idx_n_dev, sizeof(int)));
+        // (1) the MPD histogram: its non-empty bins are the distinct ray-count values
+        if (int rc = mlens_mpd(h, count_dev, h->idx_hist, (int)n_bins, cuda_stream, nullptr)) return rc;
+        // (2) compaction -> index file (values, ascending) and the count -> index table
+        mlk::index_build_kernel<<<1, 1024, 0, st>>>(h->idx_hist, (int)n_bins, h->idx_lut, values_dev, max_values, h->idx_n_dev);
+        MLENS_CUDA(cudaGetLastError());
+        // (3) ONE host round trip: the number of distinct values and whether any count was clamped
+        MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 5, h->idx_n_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
+        MLENS_CUDA(cudaMemcpyAsync(h->mapstats_host, h->mapstats_dev, sizeof(mlk::MapStatsDev), cudaMemcpyDeviceToHost, st));
+        MLENS_CUDA(cudaStreamSynchronize(st));
+        memcpy(&nd, h->counters_host + 5, sizeof(int));
+        if (h->mapstats_host->n_clamped == 0ull) break;  // every count had its own bin
+        const long long need = (long long)h->mapstats_host->max_count + 2;
+        if (need > 2147483647LL) return fail(MLENS_ERANGE, "largest count %d: the histogram would need more than 2^31-1 bins", h->mapstats_host->max_count);
+        if (attempt > 0 || need <= n_bins) return fail(MLENS_ECUDA, "mlens_index_map: histogram of %lld bins still clamps (largest count %d)", n_bins, h->mapstats_host->max_count);
+        n_bins = need;
     }
-    if (!h->idx_n_dev) MLENS_CUDA(dev_alloc(&h->idx_n_dev, sizeof(int)));
-    // (2) the MPD histogram: its non-empty bins are the distinct ray-count values
-    if (int rc = mlens_mpd(h, count_dev, h->idx_hist, (int)n_bins, cuda_stream, nullptr)) return rc;
-    // (3) compaction -> index file (values, ascending) and the count -> index table
-    mlk::index_build_kernel<<<1, 1024, 0, st>>>(h->idx_hist, (int)n_bins, h->idx_lut, values_dev, max_values, h->idx_n_dev);
-    MLENS_CUDA(cudaGetLastError());
-    MLENS_CUDA(cudaMemcpyAsync(h->counters_host + 5, h->idx_n_dev, sizeof(int), cudaMemcpyDeviceToHost, st));
-    MLENS_CUDA(cudaStreamSynchronize(st));
-    int nd;
-    memcpy(&nd, h->counters_host + 5, sizeof(int));
     *n_distinct = nd;
     if (nd > 65536) return fail(MLENS_ERANGE, "%d distinct ray-count values do not fit a 16-bit index", nd);
     if (nd > max_values) return fail(MLENS_ERANGE, "%d distinct ray-count values, values_dev holds %d", nd, max_values);
@@ -720,14 +736,18 @@ int mlens_pack_map(mlens_t* h, const void* src_dev, int src_bits, int bits, unsi
     if (src_bits != 16 && src_bits != 32) return fail(MLENS_EINVAL, "src_bits must be 16 or 32");
     if (bits < 1 || bits > src_bits) return fail(MLENS_EINVAL, "bits must be 1..src_bits");
     const long long n = (long long)h->npix * h->npix, n_words = mlens_packed_words(n, bits);
-    const long long words_per_cta = (long long)(256 / bits) * bits;  // whole 32-value periods per CTA iteration
-    long long blocks = (n_words + words_per_cta - 1) / words_per_cta;
-    if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
+    // a chunk = n_sub sub-blocks of 256/bits whole 32-value periods, at most kPackChunkValues values
+    const int vals_per_sub = (256 / bits) * 32;
+    int n_sub = mlk::kPackChunkValues / vals_per_sub;
+    if (n_sub < 1) n_sub = 1;
+    const long long chunk_vals = (long long)n_sub * vals_per_sub;
+    long long blocks = (n + chunk_vals - 1) / chunk_vals;
+    if (blocks > (long long)h->sm_count * 32) blocks = (long long)h->sm_count * 32;
     if (blocks < 1) blocks = 1;
     if (src_bits == 32)
-        mlk::pack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const int*)src_dev, n, bits, packed_dev, n_words);
+        mlk::pack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const int*)src_dev, n, bits, packed_dev, n_words, n_sub);
     else
-        mlk::pack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned short*)src_dev, n, bits, packed_dev, n_words);
+        mlk::pack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>((const unsigned short*)src_dev, n, bits, packed_dev, n_words, n_sub);
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }
@@ -742,9 +762,9 @@ int mlens_unpack_map(mlens_t* h, const unsigned int* packed_dev, int bits, void*
     if (blocks > (long long)h->sm_count * 16) blocks = (long long)h->sm_count * 16;
     if (blocks < 1) blocks = 1;
     if (dst_bits == 32)
-        mlk::unpack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (int*)dst_dev);
+        mlk::unpack_bits_kernel<int><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (int*)dst_dev, mlens_packed_words(n, bits));
     else
-        mlk::unpack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (unsigned short*)dst_dev);
+        mlk::unpack_bits_kernel<unsigned short><<<(unsigned)blocks, 256, 0, (cudaStream_t)cuda_stream>>>(packed_dev, n, bits, (unsigned short*)dst_dev, mlens_packed_words(n, bits));
     MLENS_CUDA(cudaGetLastError());
     return MLENS_OK;
 }
@@ -988,9 +1008,12 @@ extern "C" int mlens_mpd_static(const int* count_dev, long long n_pixels, double
     if (blocks > kStaticMaxCtas) blocks = kStaticMaxCtas;
     if (blocks < 1) blocks = 1;
     const size_t smem = sizeof(unsigned int) * (size_t)smem_bins;
-    MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n_pixels, hist_dev, n_bins, smem_bins, partial, st_dev);
-    MLENS_CUDA(cudaGetLastError());
+    {
+        std::lock_guard<std::mutex> launch_lock(g_launch_mutex);
+        MLENS_CUDA(cudaFuncSetAttribute(mlk::mpd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        mlk::mpd_kernel<<<(unsigned)blocks, mlk::kMpdThreads, smem, st>>>(count_dev, n_pixels, hist_dev, n_bins, smem_bins, partial, st_dev);
+        MLENS_CUDA(cudaGetLastError());
+    }
     mlk::mpd_reduce_kernel<<<(smem_bins + 31) / 32, 256, 0, st>>>(partial, (int)blocks, smem_bins, hist_dev, n_bins, st_dev);
     MLENS_CUDA(cudaGetLastError());
     if (stats) {

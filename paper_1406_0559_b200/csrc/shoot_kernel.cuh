@@ -66,7 +66,7 @@ struct ShootParams {
     unsigned long long* counters;   // [0] in_map [1] outside [2] lost [3] total
     unsigned long long* tile_counter;  // this launch's dynamic tile counter (zeroed on the launch's stream)
     int bin_mode;
-    const float* umma_A;            // kernel 3 only: the 32 ray blocks of a tile in UMMA layout (shoot_umma_kernel.cuh)
+    const float* reserved;          // unused (kept so that the parameter layout, and with it the generated code, stays as measured)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
